@@ -1,0 +1,39 @@
+"""Test helpers: build an oracle simulation from a workloads.Case (test infrastructure)."""
+import numpy as np
+
+from oracle import oracle as O
+from paper_2504_04465_b200 import workloads as W
+
+
+def oracle_from_case(case, init=True):
+    cfg = O.make_config(**case.model_kwargs())
+    g = O.OracleGrid(cfg, case.mesh.split, case.mesh.solid)
+    if init:
+        cells = [g.cells(l)[:2] for l in range(g.depth + 1)]
+        rho, ux, uy, T = W.eval_fields(case, cells)
+        rc = g.init_fields(rho, ux, uy, T)
+        assert rc == 0, "oracle init status %d" % rc
+    return g
+
+
+def level_slices(g):
+    return [slice(int(g.off[l]), int(g.off[l + 1])) for l in range(g.depth + 1)]
+
+
+def conserved_sums(g, Q_cx=None, Q_cy=None):
+    """Mass and momentum (and population energy) over non-fine-ghost, in-box cells, weighted by cell area 4^l."""
+    cx, cy, w, opp, cs2, reach = O.lattice(g.Q)
+    M = PX = PY = E = 0.0
+    for l in range(g.depth + 1):
+        ix, iy, ty, aux = g.cells(l)
+        keep = (ty == O.FLUID) | (ty == O.COARSE_GHOST)
+        f = g.populations(l, 0)[keep]
+        a = 4.0 ** l
+        M += a * f.sum()
+        PX += a * (f * cx).sum()
+        PY += a * (f * cy).sum()
+        e = (f * (cx * cx + cy * cy)).sum()
+        if g.cfg.ddf:
+            e += g.populations(l, 1)[keep].sum()
+        E += a * e
+    return np.array([M, PX, PY, E])
