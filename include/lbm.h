@@ -1,0 +1,157 @@
+/*
+ * lbm.h -- C ABI of the B200-native quadtree lattice-Boltzmann hot path
+ * (after Coreixas & Latt, arXiv 2504.04465; PAPER.md lines cited as P:<n>).
+ *
+ * The library runs, entirely in hand-written sm_100a CUDA kernels, the per-time-step fused
+ * collide-and-stream update (Eq. 30-31) over a cell-centred, Morton-ordered quadtree
+ * with int32 neighbour-list addressing (Sec. 4.3-4.4), Rohde-style coalescence /
+ * uniform explosion (Eq. 4-7) and asynchronous time stepping (listing P:202-215).
+ * The host only builds the mesh tables once.  There is no CPU fallback: every compute entry
+ * point returns LBM_ECUDA when no device is usable.
+ *
+ * Conventions
+ *  - Level 0 = finest, level `depth` = coarsest.  One coarse step = 2^depth fine steps.
+ *  - A cell of level l at integer position (ix,iy) has its centre at ((ix+1/2)h,(iy+1/2)h), h=2^l.
+ *  - Storage order of a level: in-box cells along the Z-curve with x in the even bits,
+ *    then boundary cells by (iy,ix).  Storage index = rank in that order (int32).
+ *  - Canonical direction order: index 0 = rest, then the groups of Table 4 in row order,
+ *    inside a group counter-clockwise from +x.
+ *  - State of a stored cell = POST-collision populations f*_i (Eq. 30), g*_i (Eq. 50) and the
+ *    multipliers lambda (Eq. 39) that produced them.
+ *  - All per-cell HOST arrays are flat over levels 0..depth in storage order (level l starts at
+ *    sum_{m<l} N_m) and are owned by the caller.  Host I/O is always double; conversion to the
+ *    grid's precision happens on the device.
+ *  - Ownership: the handle and the host-side mesh tables belong to the library; DEVICE memory (one
+ *    arena sized by lbm_grid_query) and the CUDA stream belong to the caller.
+ *  - Every function returns 0 on success or a negative LBM_E* code.  No exceptions cross the ABI,
+ *    no global state.  Functions taking a grid are not thread-safe on the same grid.
+ */
+#ifndef LBM_H
+#define LBM_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LBM_MAX_LEVELS 24
+#define LBM_QMAX 37
+#define LBM_NLAMBDA 8
+
+/* collision models: BGK with polynomial equilibrium (Eq. 30, 34), recursive regularised (Eq. 33-38),
+ * BGK with numerical equilibrium (Eq. 39-49) */
+enum { LBM_BGK = 0, LBM_RR = 1, LBM_NUMEQ = 2 };
+/* boundary kind per side; sides: 0 = x<0, 1 = x>=nx, 2 = y<0, 3 = y>=ny */
+enum { LBM_BC_PERIODIC = 0, LBM_BC_WALL = 1, LBM_BC_MOVING_WALL = 2, LBM_BC_INFLOW_VBB = 3,
+       LBM_BC_DIRICHLET_EQ = 4, LBM_BC_DIRICHLET_EQ_RHO_EXTRAP = 5, LBM_BC_NEUMANN = 6 };
+/* cell types */
+enum { LBM_FLUID = 0, LBM_FINE_GHOST = 1, LBM_COARSE_GHOST = 2, LBM_NEUMANN = 3, LBM_DIRICHLET = 4 };
+/* negative link values in the neighbour list */
+enum { LBM_LINK_NONE = -1, LBM_LINK_WALL = -2, LBM_LINK_VBB0 = -3 /* -3-side */ };
+/* error codes */
+enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_EMESH = -3, LBM_ECUDA = -4,
+       LBM_EUNSTABLE = -5 /* non-finite or non-positive density */,
+       LBM_ENEWTON = -6 /* Newton-Raphson did not converge */,
+       LBM_EUNSUPPORTED = -7 /* model combination has no compiled kernel */,
+       LBM_ESTATE = -8 /* call order: not bound / not initialised */ };
+
+typedef struct {
+  int lattice;        /* 9, 13, 21, 37 (Table 4) */
+  int precision;      /* 64 or 32: storage and arithmetic type of the populations */
+  int collision;      /* LBM_BGK | LBM_RR | LBM_NUMEQ */
+  int ddf;            /* 1: second distribution g, Eq. 50-51 */
+  int sensor;         /* 1: kinetic shock sensor, Eq. 52-53 */
+  int trace_eq;       /* RR only: trace of the 2nd-order non-equilibrium moments relaxed with tau=1 */
+  int depth;          /* number of levels - 1 */
+  int nx_coarse, ny_coarse;   /* box of the coarsest level, in coarsest cells */
+  int newton_max_iter;        /* P:903; S14 */
+  int bc[4];
+  double tau0;        /* relaxation time of the finest level; tau_l = 1/2 + (tau0-1/2)/2^l (Eq. 3) */
+  double T0;          /* reference temperature of numerical equilibria; polynomial models use c_s^2 */
+  double gamma;       /* specific-heat ratio of the ddf model */
+  double sensor_A;    /* Eq. 53 */
+  double newton_tol;
+  double bc_rho[4], bc_ux[4], bc_uy[4], bc_T[4];   /* imposed states per side (walls: velocity only) */
+} lbm_config;
+
+typedef struct {
+  int depth, Q, W;              /* W = lattice reach = ghost-band width in coarse cells */
+  int npop;                     /* reals per cell: Q (+Q with g) (+8 with numerical equilibria) */
+  int precision;
+  int64_t n_cells[LBM_MAX_LEVELS];        /* stored cells per level, ghosts and boundary cells included */
+  int64_t n_inbox[LBM_MAX_LEVELS];        /* of which inside the box (Morton-ordered part) */
+  int64_t n_coarse_ghosts[LBM_MAX_LEVELS];/* coarse ghosts of interface (l, l-1); 0 for l = 0 */
+  int64_t n_fine_ghosts[LBM_MAX_LEVELS];
+  int64_t n_total;                        /* sum of n_cells */
+  int64_t updates_per_coarse_step;        /* sum_l n_cells[l] * 2^(depth-l): actual cell updates */
+  int64_t launches_per_coarse_step;       /* kernels enqueued per coarse step */
+  size_t  arena_bytes;                    /* device memory the caller must provide to lbm_grid_bind */
+  double  tau[LBM_MAX_LEVELS];
+} lbm_grid_info;
+
+typedef struct lbm_grid lbm_grid;   /* opaque */
+
+/* Builds the quadtree levels, Morton order, neighbour lists, ghost lists and the level schedule on the
+ * HOST (Sec. 4.3-4.4; rules: DESIGN.md Sec. 6).  No CUDA call is made.
+ * Mesh = internal nodes + solid positions: split_xy / solid_xy are flat HOST (ix,iy) int32 pairs, the
+ * cells of level l occupy pairs [off[l], off[l+1]) (off has depth+2 entries; level 0 has no split
+ * cells); either pair of pointers may be NULL (= empty).  Returns LBM_EMESH if the mesh violates the
+ * 2:1 / ghost-band rules, LBM_EUNSUPPORTED if the model combination has no compiled kernel. */
+int lbm_grid_create(const lbm_config* cfg,
+                    const int64_t* split_off, const int32_t* split_xy,
+                    const int64_t* solid_off, const int32_t* solid_xy,
+                    lbm_grid** out);
+void lbm_destroy(lbm_grid* g);
+
+int lbm_grid_query(const lbm_grid* g, lbm_grid_info* out);
+
+/* Bit-exact tables (HOST outputs, caller-owned, any may be NULL):
+ *  cells:    ix, iy, type, aux per stored cell (aux: ghost-list index of a coarse ghost, source cell of a
+ *            Neumann / Dirichlet cell, -1 otherwise)
+ *  nbr:      n_cells*(Q-1) int32, row-major per cell: pull source of direction i (cell at x - xi_i) at
+ *            [cell*(Q-1)+i-1], or a negative LBM_LINK_* value
+ *  ghosts:   per coarse ghost of level l >= 1: its storage index, its 4 children on level l-1 in order
+ *            a+2b (-1 absent), and the Q-bit mask of unknown directions
+ *  schedule: canonical (pull) form of listing P:202-215: for fine step k = 1..2^depth the levels updated,
+ *            ascending; returns the number of entries (writes at most cap). */
+int lbm_get_cells(const lbm_grid* g, int level, int32_t* ix, int32_t* iy, int32_t* type, int32_t* aux);
+int lbm_get_nbr(const lbm_grid* g, int level, int32_t* nbr);
+int lbm_get_ghosts(const lbm_grid* g, int level, int32_t* coarse, int32_t* child, uint64_t* mask);
+int lbm_get_schedule(const lbm_grid* g, int32_t* k_of, int32_t* level_of, int cap);
+
+/* Attaches caller-owned DEVICE memory (>= arena_bytes, 256-byte aligned) and a CUDA stream
+ * (cudaStream_t passed as void*; NULL = legacy default stream), uploads the mesh tables and captures
+ * the CUDA graphs of one coarse step.  The arena must stay valid until lbm_destroy. */
+int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream);
+
+/* Sets every stored cell (ghosts included) to the equilibrium of the given macroscopic fields at its own
+ * centre, then runs the iteration-0 coupling (coalesce unknown -> collide -> explode,
+ * l = depth..1) without streaming (listing P:202-208).  rho, ux, uy, T: HOST arrays of n_total doubles
+ * (T may be NULL = T0; ignored by athermal models).  Computed on the device.  Synchronises. */
+int lbm_init_fields(lbm_grid* g, const double* rho, const double* ux, const double* uy, const double* T);
+
+/* Enqueues n_coarse_steps coarse steps (each 2^depth fine steps of the schedule above) on the bound
+ * stream and returns without synchronising. */
+int lbm_step(lbm_grid* g, int n_coarse_steps);
+/* Waits for the stream and returns the sticky device status: LBM_OK, LBM_EUNSTABLE or LBM_ENEWTON. */
+int lbm_sync(lbm_grid* g);
+
+/* rho, u (and T by Eq. 51) of every stored cell from its current populations; HOST outputs of
+ * n_total doubles, any may be NULL.  Synchronises. */
+int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double* T);
+/* Current populations of one level as HOST doubles, row-major [cell][component];
+ * which: 0 = f (Q), 1 = g (Q), 2 = lambda (8).  Synchronises. */
+int lbm_get_populations(lbm_grid* g, int level, int which, double* out);
+int lbm_set_populations(lbm_grid* g, int level, int which, const double* in);
+
+/* Device-time of the work enqueued by the last lbm_step call, in milliseconds (CUDA events recorded on
+ * the bound stream around it); synchronises.  Negative error code on failure. */
+double lbm_last_step_ms(lbm_grid* g);
+/* Name of the compiled sweep kernel this grid dispatches to (static string), for profiles. */
+const char* lbm_kernel_name(const lbm_grid* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

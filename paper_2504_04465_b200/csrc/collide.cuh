@@ -1,0 +1,348 @@
+// collide.cuh -- cell-local arithmetic of the CUDA path (rows a2-a5 of SURVEY.md Sec. 8(a)):
+// moments, polynomial equilibria (Eq. 34-36), recursive-regularised collision
+// (Eq. 33, 37-38 P:845-884), numerical equilibria (Eq. 39-49), second distribution
+// (Eq. 50-51), kinetic sensor (Eq. 52-53), BGK relaxation (Eq. 30).
+// Everything stays in registers; lattice constants are compile-time immediates (lattice.cuh).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "../../include/lbm.h"
+#include "lattice.cuh"
+
+namespace lbm {
+
+// Model constants, passed to every kernel by value.
+struct ModelParams {
+  double gamma, sensor_A, T0, newton_tol;
+  int newton_max_iter, trace_eq;
+  int bc_kind[4];
+  double bc_rho[4], bc_ux[4], bc_uy[4], bc_T[4];
+};
+
+enum { FLAG_UNSTABLE = 1, FLAG_NEWTON = 2 };
+
+template <typename T> struct Num;
+template <> struct Num<double> {
+  static __device__ __forceinline__ double tiny() { return 1e-300; }
+  static __device__ __forceinline__ double exp_(double x) { return exp(x); }
+  static __device__ __forceinline__ double sqrt_(double x) { return sqrt(x); }
+  static __device__ __forceinline__ double abs_(double x) { return fabs(x); }
+};
+template <> struct Num<float> {
+  static __device__ __forceinline__ float tiny() { return 1e-37f; }
+  static __device__ __forceinline__ float exp_(float x) { return expf(x); }
+  static __device__ __forceinline__ float sqrt_(float x) { return sqrtf(x); }
+  static __device__ __forceinline__ float abs_(float x) { return fabsf(x); }
+};
+
+// Hermite moments of the equilibrium: Eq. 36 (athermal, th = 0) and their thermal generalisation
+// about T0 = c_s^2, th = T - c_s^2 (the paper prints only the athermal ones).
+template <typename T>
+__device__ __forceinline__ void aeq_moments(T rho, T ux, T uy, T th, T (&a)[NA]) {
+  const T ux2 = ux * ux, uy2 = uy * uy;
+  a[A0] = rho;
+  a[AX] = rho * ux;
+  a[AY] = rho * uy;
+  a[AXX] = rho * (ux2 + th);
+  a[AXY] = rho * (ux * uy);
+  a[AYY] = rho * (uy2 + th);
+  a[AXXX] = rho * (ux2 * ux + T(3) * th * ux);
+  a[AXXY] = rho * (ux2 * uy + th * uy);
+  a[AXYY] = rho * (ux * uy2 + th * ux);
+  a[AYYY] = rho * (uy2 * uy + T(3) * th * uy);
+  a[AXXXX] = rho * (ux2 * ux2 + T(6) * th * ux2 + T(3) * th * th);
+  a[AXXXY] = rho * (ux2 * ux * uy + T(3) * th * ux * uy);
+  a[AXXYY] = rho * (ux2 * uy2 + th * (ux2 + uy2) + th * th);
+  a[AXYYY] = rho * (ux * uy2 * uy + T(3) * th * ux * uy);
+  a[AYYYY] = rho * (uy2 * uy2 + T(6) * th * uy2 + T(3) * th * th);
+}
+
+// f_i of Eq. 33/34 from the Hermite moments a, restricted to the basis of Table 5.
+template <int Q, typename T, int I>
+__device__ __forceinline__ T poly_i(const T (&a)[NA]) {
+  constexpr double c0 = hermite_coef(Lat<Q>::t, I, A0);
+  T s = T(c0) * a[A0];
+  static_for<1, NA>([&](auto kc) {
+    constexpr int K = decltype(kc)::value;
+    constexpr double c = hermite_coef(Lat<Q>::t, I, K);
+    if constexpr (c != 0.0) s += T(c) * a[K];
+  });
+  return s;
+}
+
+// rho, u (a2) and T by Eq. 51 (thermal models) or T0 = c_s^2 (athermal)
+template <int Q, typename T, bool THERMAL, bool DDF>
+__device__ __forceinline__ void moments(const ModelParams& p, const T (&f)[Q], const T (&g)[Q], T& rho, T& ux, T& uy, T& Tm) {
+  T r = T(0), jx = T(0), jy = T(0);
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
+    r += f[I];
+    if constexpr (cx != 0) jx += T(cx) * f[I];
+    if constexpr (cy != 0) jy += T(cy) * f[I];
+  });
+  rho = r; ux = jx / r; uy = jy / r;
+  if constexpr (!THERMAL) {
+    Tm = T(cs2_v<Q>);
+  } else {
+    T e2 = T(0);
+    static_for<0, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      constexpr int xi2 = Lat<Q>::t.cx[I] * Lat<Q>::t.cx[I] + Lat<Q>::t.cy[I] * Lat<Q>::t.cy[I];
+      if constexpr (DDF) e2 += T(xi2) * f[I] + g[I];
+      else if constexpr (xi2 != 0) e2 += T(xi2) * f[I];
+    });
+    const T Cv = DDF ? T(1.0 / (p.gamma - 1.0)) : T(1);
+    Tm = (e2 - r * (ux * ux + uy * uy)) / (T(2) * r * Cv);
+  }
+}
+
+// ------------------------------------------------------------------ numerical equilibrium
+// f_i(lambda) = rho exp[-(1 + sum_a lambda_a M_ia)] (Eq. 39 with a = rho); G_a = sum_i f_i M_ia - m_a
+template <int Q, typename T>
+__device__ __forceinline__ void numeq_eval(T rho, const T (&m)[NLAMBDA], const T (&lam)[NLAMBDA], T (&f)[Q], T (&G)[NLAMBDA]) {
+#pragma unroll
+  for (int a = 0; a < NLAMBDA; ++a) G[a] = T(0);
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    T e = T(1);
+    static_for<0, NLAMBDA>([&](auto ac) {
+      constexpr int A = decltype(ac)::value;
+      constexpr int M = monomial(Lat<Q>::t, I, A);
+      if constexpr (M != 0) e += lam[A] * T(M);
+    });
+    const T fi = rho * Num<T>::exp_(-e);
+    f[I] = fi;
+    static_for<0, NLAMBDA>([&](auto ac) {
+      constexpr int A = decltype(ac)::value;
+      constexpr int M = monomial(Lat<Q>::t, I, A);
+      if constexpr (M != 0) G[A] += fi * T(M);
+    });
+  });
+#pragma unroll
+  for (int a = 0; a < NLAMBDA; ++a) G[a] -= m[a];
+}
+
+// Newton direction: solve (-J) d = G, -J = sum_i f_i M_i M_i^T (symmetric positive definite), by Cholesky.
+// Returns false if the matrix is not positive definite.
+template <int Q, typename T>
+__device__ __forceinline__ bool newton_direction(const T (&f)[Q], const T (&G)[NLAMBDA], T (&d)[NLAMBDA]) {
+  T A[NLAMBDA][NLAMBDA];   // lower triangle used
+  static_for<0, NLAMBDA>([&](auto ac) {
+    constexpr int a = decltype(ac)::value;
+    static_for<0, a + 1>([&](auto bc) {
+      constexpr int b = decltype(bc)::value;
+      T s = T(0);
+      static_for<0, Q>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        constexpr int M = monomial(Lat<Q>::t, I, a) * monomial(Lat<Q>::t, I, b);
+        if constexpr (M != 0) s += f[I] * T(M);
+      });
+      A[a][b] = s;
+    });
+  });
+  // A = C C^T, in place; the reciprocal of the diagonal is kept in rd
+  T rd[NLAMBDA];
+  bool ok = true;
+  static_for<0, NLAMBDA>([&](auto jc) {
+    constexpr int j = decltype(jc)::value;
+    T s = A[j][j];
+    static_for<0, j>([&](auto kc) { constexpr int k = decltype(kc)::value; s -= A[j][k] * A[j][k]; });
+    if (!(s > T(0))) ok = false;
+    const T cjj = Num<T>::sqrt_(s);
+    A[j][j] = cjj;
+    rd[j] = T(1) / cjj;
+    static_for<j + 1, NLAMBDA>([&](auto ic) {
+      constexpr int i = decltype(ic)::value;
+      T t = A[i][j];
+      static_for<0, j>([&](auto kc) { constexpr int k = decltype(kc)::value; t -= A[i][k] * A[j][k]; });
+      A[i][j] = t * rd[j];
+    });
+  });
+  T y[NLAMBDA];
+  static_for<0, NLAMBDA>([&](auto ic) {
+    constexpr int i = decltype(ic)::value;
+    T t = G[i];
+    static_for<0, i>([&](auto kc) { constexpr int k = decltype(kc)::value; t -= A[i][k] * y[k]; });
+    y[i] = t * rd[i];
+  });
+  static_for<0, NLAMBDA>([&](auto rc) {
+    constexpr int i = NLAMBDA - 1 - decltype(rc)::value;
+    T t = y[i];
+    static_for<i + 1, NLAMBDA>([&](auto kc) { constexpr int k = decltype(kc)::value; t -= A[k][i] * d[k]; });
+    d[i] = t * rd[i];
+  });
+  return ok;
+}
+
+template <typename T>
+__device__ __forceinline__ T norm2sq(const T (&G)[NLAMBDA]) {
+  T s = T(0);
+#pragma unroll
+  for (int a = 0; a < NLAMBDA; ++a) s += G[a] * G[a];
+  return s;
+}
+
+// Newton-Raphson with a halving line search; deterministic rule of DESIGN.md Sec. 4 (S14):
+// iterate until sum|G_a| <= tol*rho or max_iter, then one unconditional full Newton step.
+// lam in/out; feq out.  Returns the number of Newton steps (polish included), negative on failure.
+template <int Q, typename T>
+__device__ __forceinline__ int feq_numerical(const ModelParams& p, T rho, T ux, T uy, T Tm, T (&lam)[NLAMBDA], T (&f)[Q]) {
+  const T u2 = ux * ux + uy * uy;
+  // right-hand sides of Eq. 42-49 with 2E = u^2 + 2T
+  const T m[NLAMBDA] = {rho, rho * ux, rho * uy, rho * (ux * ux + Tm), rho * ux * uy, rho * (uy * uy + Tm),
+                        rho * ux * (u2 + T(4) * Tm), rho * uy * (u2 + T(4) * Tm)};
+  T G[NLAMBDA], d[NLAMBDA], lt[NLAMBDA];
+  const T tol = T(p.newton_tol) * rho;
+  int it = 0;
+  bool converged = false, bad = false;
+  numeq_eval<Q, T>(rho, m, lam, f, G);
+  for (;;) {
+    T r1 = T(0);
+#pragma unroll
+    for (int a = 0; a < NLAMBDA; ++a) r1 += Num<T>::abs_(G[a]);
+    if (r1 <= tol) { converged = true; break; }
+    if (it >= p.newton_max_iter) break;
+    if (!newton_direction<Q, T>(f, G, d)) { bad = true; break; }
+    const T n0 = norm2sq(G);
+    T t = T(1);
+    for (;;) {
+#pragma unroll
+      for (int a = 0; a < NLAMBDA; ++a) lt[a] = lam[a] + t * d[a];
+      numeq_eval<Q, T>(rho, m, lt, f, G);
+      const T n1 = norm2sq(G);
+      if (n1 < n0 || t <= T(1.0 / 1024.0)) break;   // a NaN norm fails the first test and keeps halving
+      t *= T(0.5);
+    }
+#pragma unroll
+    for (int a = 0; a < NLAMBDA; ++a) lam[a] = lt[a];
+    ++it;
+  }
+  if (!bad) {   // polish
+    if (newton_direction<Q, T>(f, G, d)) {
+#pragma unroll
+      for (int a = 0; a < NLAMBDA; ++a) lam[a] += d[a];
+      numeq_eval<Q, T>(rho, m, lam, f, G);
+      ++it;
+    } else {
+      bad = true;
+    }
+  }
+  return (converged && !bad) ? it : -it - 1;
+}
+
+// Equilibrium of the configured model for a given macroscopic state (used by initialisation and by
+// Dirichlet cells).  THERMAL selects the T-dependent Hermite moments.
+template <int Q, typename T, int COLL, bool DDF>
+__device__ __forceinline__ int equilibrium(const ModelParams& p, T rho, T ux, T uy, T Tm, T (&lam)[NLAMBDA], T (&feq)[Q], T (&geq)[Q]) {
+  int it = 0;
+  if constexpr (COLL == LBM_NUMEQ) {
+    it = feq_numerical<Q, T>(p, rho, ux, uy, Tm, lam, feq);
+  } else {
+    T a[NA];
+    aeq_moments<T>(rho, ux, uy, DDF ? Tm - T(cs2_v<Q>) : T(0), a);
+    static_for<0, Q>([&](auto ic) { constexpr int I = decltype(ic)::value; feq[I] = poly_i<Q, T, I>(a); });
+  }
+  if constexpr (DDF) {
+    const T fac = T(2.0 / (p.gamma - 1.0) - 2.0) * Tm;   // Eq. 50: (2 C_v - D) T, D = 2
+#pragma unroll
+    for (int i = 0; i < Q; ++i) geq[i] = fac * feq[i];
+  }
+  return it;
+}
+
+// Eq. 53 with reading S10: alpha = 1 below 0.01; last case alpha = 1/tau (tau_eff = 1)
+template <typename T>
+__device__ __forceinline__ T sensor_alpha(T eps, T A, T tau) {
+  if (eps < T(0.01)) return T(1);
+  if (eps < T(0.10)) return T(1.05);
+  if (eps < T(1.00)) return A;
+  return T(1) / tau;
+}
+
+// Steps 2-5 of the cell update, in place: f, g pre-collision in, post-collision out.
+// Returns Newton iterations (0 for polynomial models, negative on failure); rho_out = pre-collision density.
+template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
+__device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T (&g)[Q], T (&lam)[NLAMBDA], T& rho_out) {
+  constexpr bool THERMAL = (COLL == LBM_NUMEQ) || DDF;
+  static_assert(!(COLL == LBM_RR && DDF), "RR is defined for the athermal models only");
+  T rho, ux, uy, Tm;
+  moments<Q, T, THERMAL, DDF>(p, f, g, rho, ux, uy, Tm);
+  rho_out = rho;
+  int it = 0;
+
+  if constexpr (COLL == LBM_NUMEQ || SENSOR) {
+    // equilibrium held in registers: Newton needs it; the sensor needs all of it before relaxing
+    T feq[Q], geq[Q];
+    it = equilibrium<Q, T, COLL, DDF>(p, rho, ux, uy, Tm, lam, feq, geq);
+    T tau_eff = tau;
+    if constexpr (SENSOR) {
+      T eps = T(0);
+#pragma unroll
+      for (int i = 0; i < Q; ++i) {
+        T den = Num<T>::abs_(feq[i]);
+        if (den < Num<T>::tiny()) den = Num<T>::tiny();
+        eps += Num<T>::abs_(f[i] - feq[i]) / den;          // Eq. 52
+      }
+      eps /= T(Q);
+      tau_eff = tau * sensor_alpha<T>(eps, T(p.sensor_A), tau);
+    }
+    const T keep = T(1) - T(1) / tau_eff;
+    static_assert(COLL != LBM_RR || !SENSOR, "sensor is instantiated for BGK-type relaxation only");
+#pragma unroll
+    for (int i = 0; i < Q; ++i) f[i] = feq[i] + keep * (f[i] - feq[i]);      // Eq. 30
+    if constexpr (DDF) {
+#pragma unroll
+      for (int i = 0; i < Q; ++i) g[i] = geq[i] + keep * (g[i] - geq[i]);
+    }
+  } else if constexpr (COLL == LBM_BGK) {
+    const T keep = T(1) - T(1) / tau;
+    T a[NA];
+    aeq_moments<T>(rho, ux, uy, DDF ? Tm - T(cs2_v<Q>) : T(0), a);
+    const T fac = DDF ? T(2.0 / (p.gamma - 1.0) - 2.0) * Tm : T(0);
+    static_for<0, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      const T fe = poly_i<Q, T, I>(a);
+      f[I] = fe + keep * (f[I] - fe);
+      if constexpr (DDF) { const T ge = fac * fe; g[I] = ge + keep * (g[I] - ge); }
+    });
+  } else {   // LBM_RR
+    const T keep = T(1) - T(1) / tau;
+    constexpr double c2 = cs2_v<Q>;
+    T ae[NA];
+    aeq_moments<T>(rho, ux, uy, T(0), ae);
+    // Pi = sum_i H_i^(2) (f_i - f_i^eq)
+    T pxx = T(0), pxy = T(0), pyy = T(0);
+    static_for<0, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
+      const T dn = f[I] - poly_i<Q, T, I>(ae);
+      pxx += T(cx * cx - c2) * dn;
+      if constexpr (cx * cy != 0) pxy += T(cx * cy) * dn;
+      pyy += T(cy * cy - c2) * dn;
+    });
+    if (p.trace_eq) {   // trace relaxes with tau = 1: only the deviatoric part survives (S7)
+      const T dev = T(0.5) * (pxx - pyy);
+      pxx = dev; pyy = -dev;
+    }
+    // Eq. 37-38 (typo of P:876 repaired, S2)
+    T an[NA];
+    an[A0] = T(0); an[AX] = T(0); an[AY] = T(0);
+    an[AXX] = pxx; an[AXY] = pxy; an[AYY] = pyy;
+    an[AXXX] = T(3) * ux * pxx;
+    an[AXXY] = T(2) * ux * pxy + uy * pxx;
+    an[AXYY] = T(2) * uy * pxy + ux * pyy;
+    an[AYYY] = T(3) * uy * pyy;
+    an[AXXXX] = T(4) * ux * an[AXXX] - T(6) * ux * ux * pxx;
+    an[AXXXY] = (T(3) * ux * an[AXXY] + uy * an[AXXX]) - T(3) * ux * ux * pxy - T(3) * ux * uy * pxx;
+    an[AXXYY] = T(2) * (ux * an[AXYY] + uy * an[AXXY]) - ux * ux * pyy - uy * uy * pxx - T(4) * ux * uy * pxy;
+    an[AXYYY] = (T(3) * uy * an[AXYY] + ux * an[AYYY]) - T(3) * uy * uy * pxy - T(3) * ux * uy * pyy;
+    an[AYYYY] = T(4) * uy * an[AYYY] - T(6) * uy * uy * pyy;
+#pragma unroll
+    for (int k = 0; k < NA; ++k) ae[k] += keep * an[k];                       // a* = a_eq + (1 - 1/tau) a_neq
+    static_for<0, Q>([&](auto ic) { constexpr int I = decltype(ic)::value; f[I] = poly_i<Q, T, I>(ae); });   // Eq. 33
+  }
+  return it;
+}
+
+}  // namespace lbm

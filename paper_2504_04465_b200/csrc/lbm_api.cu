@@ -1,0 +1,519 @@
+// lbm_api.cu -- the C ABI of include/lbm.h: device arena layout, table upload, the asynchronous
+// multilevel scheduler as CUDA graphs on one stream (row a10 of SURVEY.md Sec. 8(a); listing
+// P:202-215 in the canonical pull form of DESIGN.md Sec. 6), host I/O.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/lbm.h"
+#include "grid.hpp"
+#include "sweep.cuh"
+
+using namespace lbm;
+
+namespace {
+
+constexpr int BLOCK = 128;
+constexpr size_t ALIGN = 256;
+
+struct DevLevel {
+  int64_t n = 0, ps = 0, ng = 0;
+  size_t off_type = 0, off_aux = 0, off_nbr = 0, off_gcoarse = 0, off_gchild = 0, off_S[2] = {0, 0};
+  unsigned char* type = nullptr;
+  int* aux = nullptr;
+  int* nbr = nullptr;
+  int* g_coarse = nullptr;
+  int* g_child = nullptr;
+  void* S[2] = {nullptr, nullptr};
+  int cur = 0;
+};
+
+template <typename T>
+__global__ void export_kernel(const T* S, long long ps, int n, int comp0, int cnt, double* out) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long long)n * cnt) return;
+  const int p = (int)(t / n), c = (int)(t % n);          // coalesced reads of plane p
+  out[(long long)c * cnt + p] = (double)S[(long long)(comp0 + p) * ps + c];
+}
+
+template <typename T>
+__global__ void import_kernel(T* S, long long ps, int n, int comp0, int cnt, const double* in) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long long)n * cnt) return;
+  const int p = (int)(t / n), c = (int)(t % n);
+  S[(long long)(comp0 + p) * ps + c] = (T)in[(long long)c * cnt + p];
+}
+
+size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+struct lbm_grid {
+  HostGrid hg;
+  const KernelSet* ks = nullptr;
+  ModelParams mp;
+  int Q = 0, npop = 0, esize = 8, depth = 0;
+  std::vector<DevLevel> dl;
+  int64_t n_total = 0, launches_per_coarse = 0, updates_per_coarse = 0;
+  size_t arena_bytes = 0, off_status = 0, off_scratch = 0, scratch_doubles = 0;
+  bool bound = false, inited = false, own_stream = false;
+  char* arena = nullptr;
+  cudaStream_t stream = nullptr;
+  int* d_status = nullptr;
+  double* d_scratch = nullptr;
+  cudaGraphExec_t g1[2] = {nullptr, nullptr};     // one coarse step, starting parity of the coarsest level
+  cudaGraphExec_t gk[2] = {nullptr, nullptr};     // K coarse steps (K even), for launch-bound small grids
+  int K = 0;
+  cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+  bool timed = false;
+};
+
+namespace {
+
+#define CK(call)                                  \
+  do {                                            \
+    cudaError_t e_ = (call);                      \
+    if (e_ != cudaSuccess) return LBM_ECUDA;      \
+  } while (0)
+
+const KernelSet* find_kernel_set(const lbm_config& c) {
+  const KernelSet* sets = nullptr;
+  int n = 0;
+  switch (c.lattice) {
+    case 9: n = kernel_sets_q9(&sets); break;
+    case 13: n = kernel_sets_q13(&sets); break;
+    case 21: n = kernel_sets_q21(&sets); break;
+    case 37: n = kernel_sets_q37(&sets); break;
+    default: return nullptr;
+  }
+  for (int i = 0; i < n; ++i)
+    if (sets[i].precision == c.precision && sets[i].collision == c.collision && sets[i].ddf == (c.ddf != 0) &&
+        sets[i].sensor == (c.sensor != 0))
+      return &sets[i];
+  return nullptr;
+}
+
+int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s) {
+  if (n <= 0) return LBM_OK;
+  void* args[2] = {a0, a1};
+  const unsigned grid = (unsigned)((n + BLOCK - 1) / BLOCK);
+  CK(cudaLaunchKernel(fn, dim3(grid), dim3(BLOCK), args, 0, s));
+  return LBM_OK;
+}
+
+// One update of level l (old -> new buffer, coupling with level l-1 fused in), then flip its parity.
+int enqueue_level(lbm_grid* g, int l, int* cur) {
+  DevLevel& L = g->dl[l];
+  LevelArgs a;
+  a.n = (int)L.n; a.ps = L.ps;
+  a.So = L.S[cur[l]]; a.Sn = L.S[1 - cur[l]];
+  a.nbr = L.nbr; a.type = L.type; a.aux = L.aux; a.g_child = L.g_child;
+  a.fine = l > 0 ? g->dl[l - 1].S[cur[l - 1]] : nullptr;
+  a.fps = l > 0 ? g->dl[l - 1].ps : 0;
+  a.tau = g->hg.lv[l].tau;
+  a.status = g->d_status;
+  int rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream);
+  cur[l] ^= 1;
+  return rc;
+}
+
+// Canonical (pull) form of the listing P:202-215: fine step k = 1..2^d updates level 0, then every
+// level l with k = 0 mod 2^l, ascending.
+int enqueue_coarse_step(lbm_grid* g, int* cur) {
+  const int d = g->depth;
+  for (int64_t k = 1; k <= ((int64_t)1 << d); ++k)
+    for (int l = 0; l <= d; ++l) {
+      if (l > 0 && (k % ((int64_t)1 << l)) != 0) break;
+      int rc = enqueue_level(g, l, cur);
+      if (rc) return rc;
+    }
+  return LBM_OK;
+}
+
+int capture(lbm_grid* g, int parity, int nsteps, cudaGraphExec_t* out) {
+  std::vector<int> cur((size_t)g->depth + 1, 0);
+  cur[g->depth] = parity;
+  cudaGraph_t graph = nullptr;
+  CK(cudaStreamBeginCapture(g->stream, cudaStreamCaptureModeThreadLocal));
+  int rc = LBM_OK;
+  for (int s = 0; s < nsteps && !rc; ++s) rc = enqueue_coarse_step(g, cur.data());
+  cudaError_t e = cudaStreamEndCapture(g->stream, &graph);
+  if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+  if (e != cudaSuccess) return LBM_ECUDA;
+  e = cudaGraphInstantiate(out, graph, 0);
+  cudaGraphDestroy(graph);
+  return e == cudaSuccess ? LBM_OK : LBM_ECUDA;
+}
+
+int status_code(lbm_grid* g) {
+  int flags = 0;
+  CK(cudaMemcpyAsync(&flags, g->d_status, sizeof(int), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  if (flags & FLAG_UNSTABLE) return LBM_EUNSTABLE;
+  if (flags & FLAG_NEWTON) return LBM_ENEWTON;
+  return LBM_OK;
+}
+
+int pop_range(const lbm_grid* g, int which, int* off, int* cnt) {
+  const bool ddf = g->hg.cfg.ddf != 0, numeq = g->hg.cfg.collision == LBM_NUMEQ;
+  if (which == 0) { *off = 0; *cnt = g->Q; return LBM_OK; }
+  if (which == 1 && ddf) { *off = g->Q; *cnt = g->Q; return LBM_OK; }
+  if (which == 2 && numeq) { *off = (ddf ? 2 : 1) * g->Q; *cnt = LBM_NLAMBDA; return LBM_OK; }
+  return LBM_EINVAL;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32_t* split_xy,
+                    const int64_t* solid_off, const int32_t* solid_xy, lbm_grid** out) {
+  if (!cfg || !out) return LBM_EINVAL;
+  *out = nullptr;
+  if (cfg->precision != 64 && cfg->precision != 32) return LBM_EINVAL;
+  if (cfg->collision < LBM_BGK || cfg->collision > LBM_NUMEQ) return LBM_EINVAL;
+  if (cfg->collision == LBM_RR && cfg->ddf) return LBM_EINVAL;     // RR is defined for the athermal models only
+  if (!(cfg->tau0 >= 0.5)) return LBM_EINVAL;
+  // velocity bounce-back is defined for the weakly compressible models only
+  for (int s = 0; s < 4; ++s)
+    if ((cfg->bc[s] == LBM_BC_MOVING_WALL || cfg->bc[s] == LBM_BC_INFLOW_VBB) && (cfg->ddf || cfg->collision == LBM_NUMEQ))
+      return LBM_EINVAL;
+  Lattice lat;
+  if (!make_lattice(cfg->lattice, &lat)) return LBM_EINVAL;
+  const KernelSet* ks = find_kernel_set(*cfg);
+  if (!ks) return LBM_EUNSUPPORTED;
+  lbm_grid* g = new (std::nothrow) lbm_grid();
+  if (!g) return LBM_ENOMEM;
+  int rc = build_grid(*cfg, split_off, split_xy, solid_off, solid_xy, &g->hg);
+  if (rc) { delete g; return rc; }
+  try {
+    g->ks = ks;
+    g->Q = lat.Q;
+    g->depth = cfg->depth;
+    g->esize = cfg->precision / 8;
+    g->npop = lat.Q * (cfg->ddf ? 2 : 1) + (cfg->collision == LBM_NUMEQ ? LBM_NLAMBDA : 0);
+    ModelParams& mp = g->mp;
+    mp.gamma = cfg->gamma; mp.sensor_A = cfg->sensor_A; mp.T0 = cfg->T0; mp.newton_tol = cfg->newton_tol;
+    mp.newton_max_iter = cfg->newton_max_iter; mp.trace_eq = cfg->trace_eq;
+    for (int s = 0; s < 4; ++s) {
+      mp.bc_kind[s] = cfg->bc[s];
+      mp.bc_rho[s] = cfg->bc_rho[s]; mp.bc_ux[s] = cfg->bc_ux[s]; mp.bc_uy[s] = cfg->bc_uy[s]; mp.bc_T[s] = cfg->bc_T[s];
+    }
+    // arena layout: status word | per level: type, aux, list, ghost lists, two population buffers | scratch
+    g->dl.assign((size_t)g->depth + 1, DevLevel());
+    size_t off = 0;
+    g->off_status = off; off += ALIGN;
+    int64_t nmax = 0;
+    for (int l = 0; l <= g->depth; ++l) {
+      const HostLevel& H = g->hg.lv[l];
+      DevLevel& L = g->dl[l];
+      L.n = H.n; L.ng = H.ng;
+      L.ps = (int64_t)round_up((size_t)std::max<int64_t>(H.n, 1), 64);   // planes start on 256-byte boundaries
+      L.off_type = off; off += round_up((size_t)L.ps, ALIGN);
+      L.off_aux = off; off += round_up((size_t)L.ps * 4, ALIGN);
+      L.off_nbr = off; off += round_up((size_t)L.ps * 4 * (size_t)(g->Q - 1), ALIGN);
+      L.off_gcoarse = off; off += round_up((size_t)std::max<int64_t>(H.ng, 1) * 4, ALIGN);
+      L.off_gchild = off; off += round_up((size_t)std::max<int64_t>(H.ng, 1) * 16, ALIGN);
+      for (int b = 0; b < 2; ++b) { L.off_S[b] = off; off += round_up((size_t)L.ps * (size_t)g->npop * (size_t)g->esize, ALIGN); }
+      g->n_total += H.n;
+      nmax = std::max(nmax, H.n);
+      g->updates_per_coarse += H.n << (g->depth - l);
+      g->launches_per_coarse += (H.n > 0 ? 1 : 0) * ((int64_t)1 << (g->depth - l));
+    }
+    g->scratch_doubles = (size_t)std::max<int64_t>(4 * g->n_total, nmax * std::max(g->Q, LBM_NLAMBDA)) + 8;
+    g->off_scratch = off; off += round_up(g->scratch_doubles * 8, ALIGN);
+    g->arena_bytes = off;
+  } catch (const std::bad_alloc&) {
+    delete g;
+    return LBM_ENOMEM;
+  }
+  *out = g;
+  return LBM_OK;
+}
+
+void lbm_destroy(lbm_grid* g) {
+  if (!g) return;
+  if (g->bound) {
+    cudaStreamSynchronize(g->stream);
+    for (int p = 0; p < 2; ++p) {
+      if (g->g1[p]) cudaGraphExecDestroy(g->g1[p]);
+      if (g->gk[p]) cudaGraphExecDestroy(g->gk[p]);
+    }
+    if (g->ev0) cudaEventDestroy(g->ev0);
+    if (g->ev1) cudaEventDestroy(g->ev1);
+    if (g->own_stream) cudaStreamDestroy(g->stream);
+  }
+  delete g;
+}
+
+int lbm_grid_query(const lbm_grid* g, lbm_grid_info* o) {
+  if (!g || !o) return LBM_EINVAL;
+  memset(o, 0, sizeof(*o));
+  o->depth = g->depth; o->Q = g->Q; o->W = g->hg.lat.W; o->npop = g->npop; o->precision = g->hg.cfg.precision;
+  for (int l = 0; l <= g->depth; ++l) {
+    const HostLevel& H = g->hg.lv[l];
+    o->n_cells[l] = H.n; o->n_inbox[l] = H.n_inbox; o->n_coarse_ghosts[l] = H.ng; o->n_fine_ghosts[l] = H.n_fine_ghost;
+    o->tau[l] = H.tau;
+  }
+  o->n_total = g->n_total;
+  o->updates_per_coarse_step = g->updates_per_coarse;
+  o->launches_per_coarse_step = g->launches_per_coarse;
+  o->arena_bytes = g->arena_bytes;
+  return LBM_OK;
+}
+
+int lbm_get_cells(const lbm_grid* g, int l, int32_t* ix, int32_t* iy, int32_t* type, int32_t* aux) {
+  if (!g || l < 0 || l > g->depth) return LBM_EINVAL;
+  const HostLevel& H = g->hg.lv[l];
+  for (int64_t c = 0; c < H.n; ++c) {
+    if (ix) ix[c] = H.ix[c];
+    if (iy) iy[c] = H.iy[c];
+    if (type) type[c] = H.type[c];
+    if (aux) aux[c] = H.aux[c];
+  }
+  return LBM_OK;
+}
+
+int lbm_get_nbr(const lbm_grid* g, int l, int32_t* nbr) {
+  if (!g || !nbr || l < 0 || l > g->depth) return LBM_EINVAL;
+  const HostLevel& H = g->hg.lv[l];
+  const int Q = g->Q;
+  for (int i = 1; i < Q; ++i)
+    for (int64_t c = 0; c < H.n; ++c) nbr[c * (Q - 1) + i - 1] = H.nbr[(size_t)(i - 1) * H.n + c];
+  return LBM_OK;
+}
+
+int lbm_get_ghosts(const lbm_grid* g, int l, int32_t* coarse, int32_t* child, uint64_t* mask) {
+  if (!g || l < 1 || l > g->depth) return LBM_EINVAL;
+  const HostLevel& H = g->hg.lv[l];
+  if (coarse) memcpy(coarse, H.g_coarse.data(), sizeof(int32_t) * (size_t)H.ng);
+  if (child) memcpy(child, H.g_child.data(), sizeof(int32_t) * (size_t)(4 * H.ng));
+  if (mask) memcpy(mask, H.g_mask.data(), sizeof(uint64_t) * (size_t)H.ng);
+  return LBM_OK;
+}
+
+int lbm_get_schedule(const lbm_grid* g, int32_t* k_of, int32_t* level_of, int cap) {
+  if (!g) return LBM_EINVAL;
+  int n = 0;
+  for (int64_t k = 1; k <= ((int64_t)1 << g->depth); ++k)
+    for (int l = 0; l <= g->depth; ++l) {
+      if (l > 0 && (k % ((int64_t)1 << l)) != 0) break;
+      if (n < cap) {
+        if (k_of) k_of[n] = (int32_t)k;
+        if (level_of) level_of[n] = l;
+      }
+      ++n;
+    }
+  return n;
+}
+
+int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream) {
+  if (!g || !dev_arena) return LBM_EINVAL;
+  if (g->bound) return LBM_ESTATE;
+  if (nbytes < g->arena_bytes || ((uintptr_t)dev_arena % ALIGN) != 0) return LBM_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LBM_ECUDA;   // no CPU fallback
+  g->arena = (char*)dev_arena;
+  if (cuda_stream) {
+    g->stream = (cudaStream_t)cuda_stream;
+  } else {
+    CK(cudaStreamCreateWithFlags(&g->stream, cudaStreamNonBlocking));
+    g->own_stream = true;
+  }
+  g->d_status = (int*)(g->arena + g->off_status);
+  g->d_scratch = (double*)(g->arena + g->off_scratch);
+  CK(cudaMemsetAsync(g->d_status, 0, ALIGN, g->stream));
+  const int Q = g->Q;
+  std::vector<unsigned char> tbytes;
+  for (int l = 0; l <= g->depth; ++l) {
+    const HostLevel& H = g->hg.lv[l];
+    DevLevel& L = g->dl[l];
+    L.type = (unsigned char*)(g->arena + L.off_type);
+    L.aux = (int*)(g->arena + L.off_aux);
+    L.nbr = (int*)(g->arena + L.off_nbr);
+    L.g_coarse = (int*)(g->arena + L.off_gcoarse);
+    L.g_child = (int*)(g->arena + L.off_gchild);
+    for (int b = 0; b < 2; ++b) L.S[b] = g->arena + L.off_S[b];
+    L.cur = 0;
+    if (H.n == 0) continue;
+    tbytes.resize((size_t)H.n);
+    for (int64_t c = 0; c < H.n; ++c) tbytes[c] = (unsigned char)(H.type[c] | (H.side[c] << TYPE_SIDE_SHIFT));
+    CK(cudaMemcpyAsync(L.type, tbytes.data(), (size_t)H.n, cudaMemcpyHostToDevice, g->stream));
+    CK(cudaStreamSynchronize(g->stream));   // tbytes is reused per level
+    CK(cudaMemcpyAsync(L.aux, H.aux.data(), (size_t)H.n * 4, cudaMemcpyHostToDevice, g->stream));
+    CK(cudaMemcpy2DAsync(L.nbr, (size_t)L.ps * 4, H.nbr.data(), (size_t)H.n * 4, (size_t)H.n * 4, (size_t)(Q - 1),
+                         cudaMemcpyHostToDevice, g->stream));
+    if (H.ng > 0) {
+      CK(cudaMemcpyAsync(L.g_coarse, H.g_coarse.data(), (size_t)H.ng * 4, cudaMemcpyHostToDevice, g->stream));
+      CK(cudaMemcpyAsync(L.g_child, H.g_child.data(), (size_t)H.ng * 16, cudaMemcpyHostToDevice, g->stream));
+    }
+    // padding of the population planes is never read by a valid link; zero it once so that exports are clean
+    for (int b = 0; b < 2; ++b) CK(cudaMemsetAsync(L.S[b], 0, (size_t)L.ps * g->npop * g->esize, g->stream));
+  }
+  CK(cudaStreamSynchronize(g->stream));
+  CK(cudaEventCreate(&g->ev0));
+  CK(cudaEventCreate(&g->ev1));
+  g->bound = true;
+  // graphs: one coarse step from either parity of the coarsest level, and K steps for launch-bound grids
+  for (int p = 0; p < 2; ++p) {
+    int rc = capture(g, p, 1, &g->g1[p]);
+    if (rc) return rc;
+  }
+  g->K = 0;
+  if (g->launches_per_coarse > 0 && g->launches_per_coarse <= 32) {
+    int K = (int)(128 / g->launches_per_coarse);
+    K -= K & 1;
+    if (K >= 2) {
+      g->K = K;
+      for (int p = 0; p < 2; ++p) {
+        int rc = capture(g, p, K, &g->gk[p]);
+        if (rc) return rc;
+      }
+    }
+  }
+  return LBM_OK;
+}
+
+int lbm_init_fields(lbm_grid* g, const double* rho, const double* ux, const double* uy, const double* T) {
+  if (!g || !rho || !ux || !uy) return LBM_EINVAL;
+  if (!g->bound) return LBM_ESTATE;
+  const size_t N = (size_t)g->n_total;
+  double* d_rho = g->d_scratch;
+  double* d_ux = d_rho + N;
+  double* d_uy = d_ux + N;
+  double* d_T = d_uy + N;
+  CK(cudaMemsetAsync(g->d_status, 0, sizeof(int), g->stream));
+  CK(cudaMemcpyAsync(d_rho, rho, N * 8, cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(d_ux, ux, N * 8, cudaMemcpyHostToDevice, g->stream));
+  CK(cudaMemcpyAsync(d_uy, uy, N * 8, cudaMemcpyHostToDevice, g->stream));
+  if (T) CK(cudaMemcpyAsync(d_T, T, N * 8, cudaMemcpyHostToDevice, g->stream));
+  int64_t base = 0;
+  for (int l = 0; l <= g->depth; ++l) {
+    DevLevel& L = g->dl[l];
+    InitArgs a;
+    a.n = (int)L.n; a.ps = L.ps; a.S0 = L.S[0]; a.S1 = L.S[1];
+    a.rho = d_rho + base; a.ux = d_ux + base; a.uy = d_uy + base; a.Tin = T ? d_T + base : nullptr;
+    a.status = g->d_status;
+    int rc = launch(g->ks->init, L.n, &a, &g->mp, g->stream);
+    if (rc) return rc;
+    L.cur = 0;
+    base += L.n;
+  }
+  // coupling of iteration 0 (listing P:202-208), coarsest interface first
+  for (int l = g->depth; l >= 1; --l) {
+    DevLevel& L = g->dl[l];
+    if (L.ng == 0) continue;
+    CoupleArgs a;
+    a.ng = (int)L.ng; a.ps = L.ps; a.S = L.S[0]; a.nbr = L.nbr; a.g_coarse = L.g_coarse; a.g_child = L.g_child;
+    a.fine = g->dl[l - 1].S[0]; a.fps = g->dl[l - 1].ps; a.tau = g->hg.lv[l].tau; a.status = g->d_status;
+    int rc = launch(g->ks->couple, L.ng, &a, &g->mp, g->stream);
+    if (rc) return rc;
+  }
+  g->inited = true;
+  g->timed = false;
+  return status_code(g);
+}
+
+int lbm_step(lbm_grid* g, int n) {
+  if (!g || n < 0) return LBM_EINVAL;
+  if (!g->bound || !g->inited) return LBM_ESTATE;
+  int& p = g->dl[g->depth].cur;
+  CK(cudaEventRecord(g->ev0, g->stream));
+  while (n > 0) {
+    if (g->K >= 2 && n >= g->K) {
+      CK(cudaGraphLaunch(g->gk[p], g->stream));     // K even: parity unchanged
+      n -= g->K;
+    } else {
+      CK(cudaGraphLaunch(g->g1[p], g->stream));
+      p ^= 1;
+      n -= 1;
+    }
+  }
+  CK(cudaEventRecord(g->ev1, g->stream));
+  g->timed = true;
+  return LBM_OK;
+}
+
+int lbm_sync(lbm_grid* g) {
+  if (!g) return LBM_EINVAL;
+  if (!g->bound) return LBM_ESTATE;
+  return status_code(g);
+}
+
+double lbm_last_step_ms(lbm_grid* g) {
+  if (!g) return (double)LBM_EINVAL;
+  if (!g->bound || !g->timed) return (double)LBM_ESTATE;
+  if (cudaEventSynchronize(g->ev1) != cudaSuccess) return (double)LBM_ECUDA;
+  float ms = 0.f;
+  if (cudaEventElapsedTime(&ms, g->ev0, g->ev1) != cudaSuccess) return (double)LBM_ECUDA;
+  return (double)ms;
+}
+
+const char* lbm_kernel_name(const lbm_grid* g) { return g ? g->ks->name : ""; }
+
+int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double* T) {
+  if (!g) return LBM_EINVAL;
+  if (!g->bound || !g->inited) return LBM_ESTATE;
+  const size_t N = (size_t)g->n_total;
+  double* d[4] = {g->d_scratch, g->d_scratch + N, g->d_scratch + 2 * N, g->d_scratch + 3 * N};
+  int64_t base = 0;
+  for (int l = 0; l <= g->depth; ++l) {
+    DevLevel& L = g->dl[l];
+    MacroArgs a;
+    a.n = (int)L.n; a.ps = L.ps; a.S = L.S[L.cur];
+    a.rho = d[0] + base; a.ux = d[1] + base; a.uy = d[2] + base; a.Tm = d[3] + base;
+    int rc = launch(g->ks->macro, L.n, &a, &g->mp, g->stream);
+    if (rc) return rc;
+    base += L.n;
+  }
+  double* h[4] = {rho, ux, uy, T};
+  for (int k = 0; k < 4; ++k)
+    if (h[k]) CK(cudaMemcpyAsync(h[k], d[k], N * 8, cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return LBM_OK;
+}
+
+int lbm_get_populations(lbm_grid* g, int l, int which, double* out) {
+  if (!g || !out || l < 0 || l > g->depth) return LBM_EINVAL;
+  if (!g->bound) return LBM_ESTATE;
+  int off, cnt;
+  if (pop_range(g, which, &off, &cnt)) return LBM_EINVAL;
+  DevLevel& L = g->dl[l];
+  if (L.n == 0) return LBM_OK;
+  const long long tot = (long long)L.n * cnt;
+  const unsigned grid = (unsigned)((tot + 255) / 256);
+  if (g->esize == 8)
+    export_kernel<double><<<grid, 256, 0, g->stream>>>((const double*)L.S[L.cur], L.ps, (int)L.n, off, cnt, g->d_scratch);
+  else
+    export_kernel<float><<<grid, 256, 0, g->stream>>>((const float*)L.S[L.cur], L.ps, (int)L.n, off, cnt, g->d_scratch);
+  CK(cudaGetLastError());
+  CK(cudaMemcpyAsync(out, g->d_scratch, (size_t)tot * 8, cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return LBM_OK;
+}
+
+int lbm_set_populations(lbm_grid* g, int l, int which, const double* in) {
+  if (!g || !in || l < 0 || l > g->depth) return LBM_EINVAL;
+  if (!g->bound) return LBM_ESTATE;
+  int off, cnt;
+  if (pop_range(g, which, &off, &cnt)) return LBM_EINVAL;
+  DevLevel& L = g->dl[l];
+  if (L.n == 0) return LBM_OK;
+  const long long tot = (long long)L.n * cnt;
+  const unsigned grid = (unsigned)((tot + 255) / 256);
+  CK(cudaMemcpyAsync(g->d_scratch, in, (size_t)tot * 8, cudaMemcpyHostToDevice, g->stream));
+  if (g->esize == 8)
+    import_kernel<double><<<grid, 256, 0, g->stream>>>((double*)L.S[L.cur], L.ps, (int)L.n, off, cnt, g->d_scratch);
+  else
+    import_kernel<float><<<grid, 256, 0, g->stream>>>((float*)L.S[L.cur], L.ps, (int)L.n, off, cnt, g->d_scratch);
+  CK(cudaGetLastError());
+  CK(cudaStreamSynchronize(g->stream));
+  g->inited = true;
+  return LBM_OK;
+}
+
+}  // extern "C"

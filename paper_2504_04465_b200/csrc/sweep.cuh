@@ -1,0 +1,428 @@
+// sweep.cuh -- the level sweep of the CUDA path: one fused kernel per level update
+// (rows a1, a6-a9 of SURVEY.md Sec. 8(a) around the cell-local arithmetic of collide.cuh).
+//
+// One thread updates one cell (pull scheme, Eq. 31): it reads its Q-1 links from the
+// direction-major int32 list (coalesced), gathers Q (2Q) populations from the level's old buffer,
+// resolves wall / velocity-bounce-back links from its own old populations, and
+//   FLUID / NEUMANN   collides and stores to its own slot of the new buffer (coalesced);
+//   COARSE_GHOST      first coalesces its unknown directions from its children's current values
+//                     (Eq. 4, 6 P:104-118), collides once (S15), stores, and explodes the result to
+//                     its <= 4 children on the finer level (Eq. 5, 7 P:108-122);
+//   FINE_GHOST        stores what it gathered, without colliding;
+//   DIRICHLET         stores the equilibrium of the imposed state.
+// Each thread writes only its own slot (and its own children), so there are no atomics and no
+// write hazards; the two-buffer scheme of the paper is kept.
+#pragma once
+#include "collide.cuh"
+
+namespace lbm {
+
+constexpr int TYPE_MASK = 7;     // low bits of the device type byte = LBM_* cell type
+constexpr int TYPE_SIDE_SHIFT = 4;  // boundary cells: side in bits 4-5
+
+// Kernel arguments are plain structs with untyped pointers (the precision is a template parameter of
+// the kernel, not of its arguments), so that the host side launches every instantiation the same way.
+struct LevelArgs {
+  int n;                    // stored cells of this level
+  long long ps;             // plane stride of the population arrays and of the list (elements)
+  const void* So;           // old buffer  [npop][ps]
+  void* Sn;                 // new buffer
+  const int* nbr;           // [(Q-1)][ps] pull sources / negative link codes
+  const unsigned char* type;
+  const int* aux;           // ghost index (coarse ghost) / source cell (boundary cells)
+  const int* g_child;       // [ng][4] children on the finer level
+  void* fine;               // finer level's CURRENT buffer (coalescence reads, explosion writes)
+  long long fps;            // its plane stride
+  double tau;
+  int* status;              // sticky FLAG_* word
+};
+
+template <int Q, bool DDF, int COLL>
+struct PopLayout {
+  static constexpr int G0 = Q;                                    // first plane of g
+  static constexpr int L0 = (DDF ? 2 : 1) * Q;                    // first plane of lambda
+  static constexpr int NPOP = L0 + (COLL == LBM_NUMEQ ? NLAMBDA : 0);
+};
+
+template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
+__global__ void __launch_bounds__(128) sweep_kernel(const LevelArgs a, const ModelParams p) {
+  using PL = PopLayout<Q, DDF, COLL>;
+  constexpr bool NUMEQ = COLL == LBM_NUMEQ;
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= a.n) return;
+  const int tb = a.type[c];
+  const int type = tb & TYPE_MASK;
+  const T* __restrict__ So = (const T*)a.So;
+  T* __restrict__ Sn = (T*)a.Sn;
+  const long long ps = a.ps;
+  T f[Q], g[Q], lam[NLAMBDA];
+
+  if (type == LBM_DIRICHLET) {
+    // equilibrium Dirichlet cell: imposed (rho,u,T); rho optionally from the nearest interior cell
+    const int side = tb >> TYPE_SIDE_SHIFT;
+    T rho = T(p.bc_rho[side]);
+    if (p.bc_kind[side] == LBM_BC_DIRICHLET_EQ_RHO_EXTRAP) {
+      const int s = a.aux[c];
+      rho = T(0);
+#pragma unroll
+      for (int i = 0; i < Q; ++i) rho += So[i * ps + s];
+    }
+    const T Tb = (NUMEQ || DDF) ? T(p.bc_T[side]) : T(cs2_v<Q>);
+    if constexpr (NUMEQ) {
+#pragma unroll
+      for (int k = 0; k < NLAMBDA; ++k) lam[k] = So[(PL::L0 + k) * ps + c];
+    }
+    const int it = equilibrium<Q, T, COLL, DDF>(p, rho, T(p.bc_ux[side]), T(p.bc_uy[side]), Tb, lam, f, g);
+#pragma unroll
+    for (int i = 0; i < Q; ++i) Sn[i * ps + c] = f[i];
+    if constexpr (DDF) {
+#pragma unroll
+      for (int i = 0; i < Q; ++i) Sn[(PL::G0 + i) * ps + c] = g[i];
+    }
+    if constexpr (NUMEQ) {
+#pragma unroll
+      for (int k = 0; k < NLAMBDA; ++k) Sn[(PL::L0 + k) * ps + c] = lam[k];
+    }
+    if (it < 0) atomicOr(a.status, FLAG_NEWTON);
+    if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+    return;
+  }
+
+  // a NEUMANN cell replicates the complete update of its source cell (reading S13)
+  const int self = (type == LBM_NEUMANN) ? a.aux[c] : c;
+
+  // ---- step 1: gather (pull form of Eq. 31).  Links first (coalesced, independent loads) ...
+  int nb[Q];
+  nb[0] = self;
+  bool special = false;     // any velocity-bounce-back or (coarse ghost) unknown link
+  static_for<1, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    nb[I] = a.nbr[(long long)(I - 1) * ps + c];
+    special |= (nb[I] <= LBM_LINK_VBB0) || (nb[I] == LBM_LINK_NONE);
+  });
+  // ... then the populations, branch-free: a wall link reads the cell's own opposite population
+  // (half-way bounce-back), a NONE link the cell's own value (fine ghosts, S6; fixed up below
+  // for coarse ghosts), any other link the neighbour's.
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int O = Lat<Q>::t.opp[I];
+    const int n = nb[I];
+    const int src = n >= 0 ? n : self;
+    const int comp = (n >= 0 || n == LBM_LINK_NONE) ? I : O;
+    f[I] = So[comp * ps + src];
+    if constexpr (DDF) g[I] = So[(PL::G0 + comp) * ps + src];
+  });
+
+  if (special) {
+    if (type == LBM_COARSE_GHOST) {
+      // coalescence (Eq. 4): unknown directions only, mean over the children that exist
+      const int* ch = a.g_child + 4ll * a.aux[c];
+      const int c0 = ch[0], c1 = ch[1], c2 = ch[2], c3 = ch[3];
+      const T nf = T((c0 >= 0) + (c1 >= 0) + (c2 >= 0) + (c3 >= 0));
+      const T* F = (const T*)a.fine;
+      const long long fps = a.fps;
+      static_for<1, Q>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        if (nb[I] == LBM_LINK_NONE) {
+          T s = T(0);
+          if (c0 >= 0) s += F[I * fps + c0];
+          if (c1 >= 0) s += F[I * fps + c1];
+          if (c2 >= 0) s += F[I * fps + c2];
+          if (c3 >= 0) s += F[I * fps + c3];
+          f[I] = s / nf;
+          if constexpr (DDF) {
+            T sg = T(0);
+            if (c0 >= 0) sg += F[(PL::G0 + I) * fps + c0];
+            if (c1 >= 0) sg += F[(PL::G0 + I) * fps + c1];
+            if (c2 >= 0) sg += F[(PL::G0 + I) * fps + c2];
+            if (c3 >= 0) sg += F[(PL::G0 + I) * fps + c3];
+            g[I] = sg / nf;
+          }
+        }
+      });
+    }
+    // velocity bounce-back (Ladd): + 2 w_i rho_w (xi_i . u_w) / c_s^2, rho_w local (S11)
+    bool vbb = false;
+    static_for<1, Q>([&](auto ic) { vbb |= nb[decltype(ic)::value] <= LBM_LINK_VBB0; });
+    if (vbb) {
+      T rho_w = T(0);
+#pragma unroll
+      for (int j = 0; j < Q; ++j) rho_w += So[j * ps + self];
+      static_for<1, Q>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        if (nb[I] <= LBM_LINK_VBB0) {
+          const int side = LBM_LINK_VBB0 - nb[I];
+          constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
+          constexpr double w2 = 2.0 * Lat<Q>::t.w[I];
+          const T xu = T(cx) * T(p.bc_ux[side]) + T(cy) * T(p.bc_uy[side]);
+          f[I] += T(w2) * rho_w * xu / T(cs2_v<Q>);
+        }
+      });
+    }
+  }
+
+  if (type == LBM_FINE_GHOST) {
+    // fine ghost cells stream without colliding; lambda stays
+#pragma unroll
+    for (int i = 0; i < Q; ++i) Sn[i * ps + c] = f[i];
+    if constexpr (DDF) {
+#pragma unroll
+      for (int i = 0; i < Q; ++i) Sn[(PL::G0 + i) * ps + c] = g[i];
+    }
+    if constexpr (NUMEQ) {
+#pragma unroll
+      for (int k = 0; k < NLAMBDA; ++k) Sn[(PL::L0 + k) * ps + c] = So[(PL::L0 + k) * ps + c];
+    }
+    return;
+  }
+
+  if constexpr (NUMEQ) {
+    if (type == LBM_COARSE_GHOST) {   // Eq. 6: warm start from the mean of the children's multipliers
+      const int* ch = a.g_child + 4ll * a.aux[c];
+      int nf = 0;
+#pragma unroll
+      for (int k = 0; k < NLAMBDA; ++k) lam[k] = T(0);
+      for (int j = 0; j < 4; ++j) {
+        const int cj = ch[j];
+        if (cj < 0) continue;
+        ++nf;
+#pragma unroll
+        for (int k = 0; k < NLAMBDA; ++k) lam[k] += ((const T*)a.fine)[(PL::L0 + k) * a.fps + cj];
+      }
+#pragma unroll
+      for (int k = 0; k < NLAMBDA; ++k) lam[k] /= T(nf);
+    } else {
+#pragma unroll
+      for (int k = 0; k < NLAMBDA; ++k) lam[k] = So[(PL::L0 + k) * ps + self];
+    }
+  }
+
+  // ---- steps 2-5: moments, equilibrium, sensor, relaxation
+  T rho;
+  const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f, g, lam, rho);
+
+  // ---- store (coalesced: own slot of the new buffer)
+#pragma unroll
+  for (int i = 0; i < Q; ++i) Sn[i * ps + c] = f[i];
+  if constexpr (DDF) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) Sn[(PL::G0 + i) * ps + c] = g[i];
+  }
+  if constexpr (NUMEQ) {
+#pragma unroll
+    for (int k = 0; k < NLAMBDA; ++k) Sn[(PL::L0 + k) * ps + c] = lam[k];
+  }
+  if (it < 0) atomicOr(a.status, FLAG_NEWTON);
+  if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+
+  if (type == LBM_COARSE_GHOST) {
+    // uniform explosion (Eq. 5, 7): every child receives the coarse post-collision state, all directions (S8)
+    const int* ch = a.g_child + 4ll * a.aux[c];
+    T* F = (T*)a.fine;
+    const long long fps = a.fps;
+    for (int j = 0; j < 4; ++j) {
+      const int cj = ch[j];
+      if (cj < 0) continue;
+#pragma unroll
+      for (int i = 0; i < Q; ++i) F[i * fps + cj] = f[i];
+      if constexpr (DDF) {
+#pragma unroll
+        for (int i = 0; i < Q; ++i) F[(PL::G0 + i) * fps + cj] = g[i];
+      }
+      if constexpr (NUMEQ) {
+#pragma unroll
+        for (int k = 0; k < NLAMBDA; ++k) F[(PL::L0 + k) * fps + cj] = lam[k];
+      }
+    }
+  }
+}
+
+// ------------------------------------------------------------------ initialisation
+struct InitArgs {
+  int n;
+  long long ps;
+  void* S0; void* S1;
+  const double* rho; const double* ux; const double* uy; const double* Tin;   // this level's slice; Tin may be null
+  int* status;
+};
+
+template <int Q, typename T, int COLL, bool DDF>
+__global__ void __launch_bounds__(128) init_kernel(const InitArgs a, const ModelParams p) {
+  using PL = PopLayout<Q, DDF, COLL>;
+  constexpr bool NUMEQ = COLL == LBM_NUMEQ;
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= a.n) return;
+  const T r = T(a.rho[c]), vx = T(a.ux[c]), vy = T(a.uy[c]);
+  const T T0 = NUMEQ ? T(p.T0) : T(cs2_v<Q>);
+  const T Tc = (NUMEQ || DDF) ? (a.Tin ? T(a.Tin[c]) : T0) : T0;
+  T f[Q], g[Q], lam[NLAMBDA];
+  if constexpr (NUMEQ) {
+    // exponents of the continuous Maxwellian as the Newton start
+    lam[0] = (vx * vx + vy * vy) / (T(2) * Tc) + T(log(2.0 * 3.14159265358979323846 * (double)Tc)) - T(1);
+    lam[1] = -vx / Tc; lam[2] = -vy / Tc; lam[3] = T(1) / (T(2) * Tc); lam[4] = T(0); lam[5] = T(1) / (T(2) * Tc);
+    lam[6] = T(0); lam[7] = T(0);
+  }
+  const int it = equilibrium<Q, T, COLL, DDF>(p, r, vx, vy, Tc, lam, f, g);
+  T* S0 = (T*)a.S0;
+  T* S1 = (T*)a.S1;
+#pragma unroll
+  for (int i = 0; i < Q; ++i) { S0[i * a.ps + c] = f[i]; S1[i * a.ps + c] = f[i]; }
+  if constexpr (DDF) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) { S0[(PL::G0 + i) * a.ps + c] = g[i]; S1[(PL::G0 + i) * a.ps + c] = g[i]; }
+  }
+  if constexpr (NUMEQ) {
+#pragma unroll
+    for (int k = 0; k < NLAMBDA; ++k) { S0[(PL::L0 + k) * a.ps + c] = lam[k]; S1[(PL::L0 + k) * a.ps + c] = lam[k]; }
+  }
+  if (it < 0) atomicOr(a.status, FLAG_NEWTON);
+  T s = T(0);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) s += f[i];
+  if (!(s > T(0)) || !isfinite(s)) atomicOr(a.status, FLAG_UNSTABLE);
+}
+
+// Coupling of iteration 0 without streaming (listing P:202-208): per coarse ghost, coalesce the unknown
+// directions from the children, collide, store in place, explode.
+struct CoupleArgs {
+  int ng;
+  long long ps;
+  void* S;                  // the coarse level's current buffer (in place)
+  const int* nbr;
+  const int* g_coarse;
+  const int* g_child;
+  void* fine; long long fps;
+  double tau;
+  int* status;
+};
+
+template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
+__global__ void __launch_bounds__(128) init_coupling_kernel(const CoupleArgs a, const ModelParams p) {
+  using PL = PopLayout<Q, DDF, COLL>;
+  constexpr bool NUMEQ = COLL == LBM_NUMEQ;
+  T* S = (T*)a.S;
+  T* fine = (T*)a.fine;
+  const int q = blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= a.ng) return;
+  const int c = a.g_coarse[q];
+  const int* ch = a.g_child + 4ll * q;
+  int nf = 0;
+  for (int j = 0; j < 4; ++j) nf += ch[j] >= 0;
+  T f[Q], g[Q], lam[NLAMBDA];
+  f[0] = S[c];
+  if constexpr (DDF) g[0] = S[PL::G0 * a.ps + c];
+  static_for<1, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    if (a.nbr[(long long)(I - 1) * a.ps + c] == LBM_LINK_NONE) {
+      T s = T(0);
+      [[maybe_unused]] T sg = T(0);
+      for (int j = 0; j < 4; ++j) {
+        if (ch[j] < 0) continue;
+        s += fine[I * a.fps + ch[j]];
+        if constexpr (DDF) sg += fine[(PL::G0 + I) * a.fps + ch[j]];
+      }
+      f[I] = s / T(nf);
+      if constexpr (DDF) g[I] = sg / T(nf);
+    } else {
+      f[I] = S[I * a.ps + c];
+      if constexpr (DDF) g[I] = S[(PL::G0 + I) * a.ps + c];
+    }
+  });
+  if constexpr (NUMEQ) {
+#pragma unroll
+    for (int k = 0; k < NLAMBDA; ++k) {
+      T s = T(0);
+      for (int j = 0; j < 4; ++j)
+        if (ch[j] >= 0) s += fine[(PL::L0 + k) * a.fps + ch[j]];
+      lam[k] = s / T(nf);
+    }
+  }
+  T rho;
+  const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f, g, lam, rho);
+  if (it < 0) atomicOr(a.status, FLAG_NEWTON);
+  if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) S[i * a.ps + c] = f[i];
+  if constexpr (DDF) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) S[(PL::G0 + i) * a.ps + c] = g[i];
+  }
+  if constexpr (NUMEQ) {
+#pragma unroll
+    for (int k = 0; k < NLAMBDA; ++k) S[(PL::L0 + k) * a.ps + c] = lam[k];
+  }
+  for (int j = 0; j < 4; ++j) {
+    const int cj = ch[j];
+    if (cj < 0) continue;
+#pragma unroll
+    for (int i = 0; i < Q; ++i) fine[i * a.fps + cj] = f[i];
+    if constexpr (DDF) {
+#pragma unroll
+      for (int i = 0; i < Q; ++i) fine[(PL::G0 + i) * a.fps + cj] = g[i];
+    }
+    if constexpr (NUMEQ) {
+#pragma unroll
+      for (int k = 0; k < NLAMBDA; ++k) fine[(PL::L0 + k) * a.fps + cj] = lam[k];
+    }
+  }
+}
+
+// rho, u, T of every cell of one level from its current populations (Eq. 51)
+struct MacroArgs {
+  int n;
+  long long ps;
+  const void* S;
+  double* rho; double* ux; double* uy; double* Tm;
+};
+
+template <int Q, typename T, int COLL, bool DDF>
+__global__ void __launch_bounds__(128) macroscopic_kernel(const MacroArgs a, const ModelParams p) {
+  using PL = PopLayout<Q, DDF, COLL>;
+  constexpr bool THERMAL = (COLL == LBM_NUMEQ) || DDF;
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= a.n) return;
+  const T* S = (const T*)a.S;
+  T f[Q], g[Q];
+#pragma unroll
+  for (int i = 0; i < Q; ++i) f[i] = S[i * a.ps + c];
+  if constexpr (DDF) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) g[i] = S[(PL::G0 + i) * a.ps + c];
+  }
+  T rho, ux, uy, Tm;
+  moments<Q, T, THERMAL, DDF>(p, f, g, rho, ux, uy, Tm);
+  a.rho[c] = (double)rho; a.ux[c] = (double)ux; a.uy[c] = (double)uy; a.Tm[c] = (double)Tm;
+}
+
+// ------------------------------------------------------------------ dispatch table entry
+struct KernelSet {
+  int Q, precision, collision, ddf, sensor;
+  const char* name;
+  const void* sweep;
+  const void* init;
+  const void* couple;
+  const void* macro;
+};
+
+template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
+KernelSet make_kernel_set(const char* name) {
+  KernelSet k;
+  k.Q = Q; k.precision = (int)sizeof(T) * 8; k.collision = COLL; k.ddf = DDF; k.sensor = SENSOR;
+  k.name = name;
+  k.sweep = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR>;
+  k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;
+  k.couple = (const void*)&init_coupling_kernel<Q, T, COLL, DDF, SENSOR>;
+  k.macro = (const void*)&macroscopic_kernel<Q, T, COLL, DDF>;
+  return k;
+}
+
+#define LBM_KSET(Q, T, COLL, DDF, SENSOR) \
+  make_kernel_set<Q, T, COLL, DDF, SENSOR>("sweep_kernel<" #Q "," #T "," #COLL "," #DDF "," #SENSOR ">")
+
+// defined one per lattice (sweep_q*.cu) so that the instantiations compile in parallel
+int kernel_sets_q9(const KernelSet** out);
+int kernel_sets_q13(const KernelSet** out);
+int kernel_sets_q21(const KernelSet** out);
+int kernel_sets_q37(const KernelSet** out);
+
+}  // namespace lbm
