@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the quadtree-LBM hot path on B200 (contract: one JSON line on stdout, rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--precision 64|32]
+    python bench.py --impl reference ...          # the CPU oracle as it stands, timed on the host cores
+
+A "step" is one pass of the whole hot path over the workload: one COARSE step = 2^depth fine steps of the
+asynchronous schedule (every level sweep with its fused coalescence / explosion / boundary links), replayed
+as a CUDA graph.  `value` = actual cell updates / s (MLUPS) with the state resident in HBM; `e2e` = the
+same through the C-ABI calls with pinned HOST buffers (lbm_init_fields H2D + lbm_step + lbm_get_macroscopic
+D2H inside the timed region, every step).  N > 1: independent replicas, one per rank (the path does not
+shard: DESIGN.md "replicas only"), no data-path collective; value = sum over ranks / max time.
+
+Workloads (synthetic, seeded, shaped like the paper's cases):
+  cylinder  BASELINE configs[2]: D2Q9-RR, 6 levels, ~9.85 M cells (default: the multilevel headline)
+  uniform   configs[0] scaled to 4096^2 (tree-stored uniform periodic D2Q9-BGK; the 80 %-of-HBM target)
+  cavity    configs[1] as given (39 k cells, launch-latency-bound)    cavity8: the same x8
+  riemann   configs[3]: D2Q37 polynomial + g + sensor, 2048^2
+  naca      configs[4]: D2Q21 numerical equilibrium + g + sensor, 7 levels, ~18 M cells
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2504_04465_b200 import workloads as W   # input generators only (no arithmetic of the method)
+
+FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+
+
+def make_case(name, scale):
+    if name == "cylinder":
+        D = int(round(200 * scale))
+        return W.cylinder(D=D), dict(workload="cylinder (BASELINE configs[2]): D2Q9-RR, D=%d, 64Dx64D, 6 levels" % D, steps=20)
+    if name == "uniform":
+        n = int(round(4096 * scale))
+        return W.tgv(n), dict(workload="uniform periodic %dx%d tree-stored D2Q9-BGK Taylor-Green (configs[0] scaled)" % (n, n), steps=200)
+    if name == "cavity":
+        return W.cavity(scale), dict(workload="cavity (BASELINE configs[1]): D2Q9-RR, 2 levels, coarse %d^2" % int(128 * scale), steps=2000)
+    if name == "cavity8":
+        return W.cavity(8 * scale), dict(workload="cavity x8: D2Q9-RR, 2 levels, coarse %d^2" % int(1024 * scale), steps=200)
+    if name == "riemann":
+        n = int(round(2048 * scale))
+        return W.riemann(n=n), dict(workload="riemann (BASELINE configs[3]): D2Q37 polynomial+g+sensor, %d^2, Neumann box" % n, steps=50)
+    if name == "naca":
+        c = int(round(1024 * scale))
+        return W.naca(chord=c), dict(workload="naca (BASELINE configs[4]): D2Q21 numerical eq.+g+sensor, chord %d, 7 levels" % c, steps=3)
+    raise SystemExit("unknown workload %r" % name)
+
+
+def algorithmic_bytes_per_update(case, precision):
+    """Two-buffer pull update with an int32 list and a type byte:
+    2*npop*s + (Q-1)*4 + 4 per cell update."""
+    Q = case.lattice
+    npop = Q * (2 if case.ddf else 1) + (8 if case.collision == W.NUMEQ else 0)
+    return 2 * npop * (precision // 8) + (Q - 1) * 4 + 4
+
+
+def fine_equivalent_cells(case):
+    m = case.mesh
+    n = m.nx_coarse * m.ny_coarse * 4 ** m.depth
+    for l, s in enumerate(m.solid):
+        n -= len(s) * 4 ** l
+    return n
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return {"hbm_gbs": FALLBACK_HBM_GBS}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out = self.p.communicate(timeout=5)[0]
+        except Exception:
+            self.p.kill()
+            out = ""
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.strip().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for k, nme in enumerate(names):
+                if c[3 + k].lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------- oracle legs (CPU)
+def oracle_grid(case):
+    from oracle import oracle as O      # test infrastructure: only these two legs of bench.py may load it
+    o = O.OracleGrid(O.make_config(**case.model_kwargs()), case.mesh.split, case.mesh.solid)
+    cells = [o.cells(l)[:2] for l in range(o.depth + 1)]
+    assert o.init_fields(*W.eval_fields(case, cells)) == 0
+    return o
+
+
+def oracle_rate(o, budget_s, min_fine_steps=1):
+    """Times the oracle, single-threaded, fine step by fine step until `budget_s` is spent; MLUPS (actual)."""
+    u0 = o.cell_updates()
+    t0 = time.perf_counter()
+    n = 0
+    while True:
+        o.step_fine(1)
+        n += 1
+        dt = time.perf_counter() - t0
+        if n >= min_fine_steps and dt >= budget_s:
+            break
+    return (o.cell_updates() - u0) / dt / 1e6, n, o.cell_updates() - u0, dt
+
+
+def run_reference(args, case, info):
+    """--impl reference: the oracle as it stands on the host cores; each step = one fine step of the schedule on
+    the full grid (a bounded sample of the coarse step the CUDA arm times)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    o = oracle_grid(case)
+    for _ in range(args.warmup):
+        o.step_fine(1)
+    u0 = o.cell_updates()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step_fine(1)
+    dt = time.perf_counter() - t0
+    upd = o.cell_updates() - u0
+    v = upd / dt / 1e6
+    sample = "%d fine steps of the schedule on the full grid (%d cell updates)" % (args.steps, upd)
+    line = {"impl": "reference", "metric": "MLUPS (actual cell updates per second)", "value": v, "unit": "MLUPS", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": dict(workload=info["workload"], precision=64),
+            "cpu_baseline": {"value": v, "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- CUDA arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="cylinder")
+    ap.add_argument("--precision", type=int, default=64, choices=[32, 64])
+    ap.add_argument("--scale", type=float, default=1.0, help="linear scale of the workload (1 = BASELINE size)")
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0, help="0 disables the cpu_baseline leg")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    args = ap.parse_args()
+    case, info = make_case(args.workload, args.scale)
+    if args.steps is None:
+        args.steps = info["steps"] if args.impl == "cuda" else 20
+    if args.impl == "reference":
+        return run_reference(args, case, info)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2504_04465_b200 import lbm     # raises if the CUDA library is not built: no fallback
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    t_build = time.perf_counter()
+    g = lbm.Grid.from_case(case, precision=args.precision)
+    g.bind(dev)
+    ntot = g.ntot
+    pin = lambda: torch.empty(ntot, dtype=torch.float64).pin_memory().numpy()
+    h_in = [pin() for _ in range(4)]
+    h_out = [pin() for _ in range(4)]
+    cells = [g.cells(l)[:2] for l in range(g.depth + 1)]
+    for dst, src in zip(h_in, W.eval_fields(case, cells)):
+        dst[:] = src
+    rc = g.init_fields(*h_in)
+    assert rc == 0, "lbm_init_fields status %d" % rc
+    t_build = time.perf_counter() - t_build
+
+    upd = int(g.info.updates_per_coarse_step)
+    launches = int(g.info.launches_per_coarse_step)
+    # ---- device-resident throughput: W warm-up steps, then exactly K steps between CUDA events on the bound stream
+    g.step(args.warmup)
+    assert g.sync() == 0
+    barrier()
+    clk = ClockSampler(local)
+    t0 = time.perf_counter()
+    g.step(args.steps)
+    ms = g.last_step_ms()            # events recorded on the grid's stream around the K graph replays; synchronises
+    status = g.sync()
+    barrier()
+    wall = time.perf_counter() - t0
+    clocks = clk.stop()
+    assert status == 0, "device status %d after the timed region" % status
+
+    # ---- end to end through the C ABI with pinned host buffers, every step: H2D fields -> step -> D2H macroscopic
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2e_ms = 0.0
+    with torch.cuda.stream(g.stream):
+        for it in range(args.e2e_steps + 1):
+            barrier()
+            ev0.record(g.stream)
+            rc = g.init_fields(*h_in)
+            g.step(1)
+            g.macroscopic(out=h_out)
+            ev1.record(g.stream)
+            ev1.synchronize()
+            assert rc == 0
+            if it > 0:               # first pass is the warm-up
+                e2e_ms += ev0.elapsed_time(ev1)
+    e2e_ms /= max(args.e2e_steps, 1)
+
+    t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, e2e_ms = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    K = args.steps
+    total_upd = upd * K * world
+    mlups = total_upd / (ms * 1e-3) / 1e6
+    bpu = algorithmic_bytes_per_update(case, args.precision)
+    peaks, peak_src = measured_peaks()
+    peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
+    achieved = upd * K * bpu / (ms * 1e-3) / 1e9          # this rank's kernel: all launches of the region are the sweep kernel
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per cell update from the committed ncu capture
+    if os.path.exists(tp):
+        try:
+            traffic = json.load(open(tp)).get("%s_f%d" % (args.workload, args.precision))
+        except Exception:
+            traffic = None
+    n_all = ntot
+    depth = g.depth
+    line = {
+        "metric": "MLUPS (actual cell updates per second)", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K,
+        "warmup": args.warmup, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f%d" % args.precision, "data": "synthetic",
+        "config": dict(workload=info["workload"], precision=args.precision, cells=n_all, levels=depth + 1,
+                       cells_per_level=g.n, updates_per_step=upd, step="one coarse step = %d fine steps" % (1 << depth),
+                       parallelism="replicas x%d" % world, l2="inputs larger than L2 (state %.0f MB)" % (g.info.arena_bytes / 1e6)
+                       if g.info.arena_bytes > 4 * 126e6 else "working set %.0f MB fits L2: launch-latency-bound case, no flush" % (g.info.arena_bytes / 1e6),
+                       kernel=g.kernel_name()),
+        "mlups": {"actual": mlups, "paper_eq13": n_all * (1 << depth) * K * world / (ms * 1e-3) / 1e6,
+                  "fine_equivalent": fine_equivalent_cells(case) * (1 << depth) * K * world / (ms * 1e-3) / 1e6},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic, "peak_source": peak_src, "bytes_per_update": bpu,
+                     "frac_of_nominal_8TBs": achieved / 8000.0},
+        "e2e": {"value": upd * world / (e2e_ms * 1e-3) / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 4 * 8 * ntot,
+                "d2h_bytes_per_step": 4 * 8 * ntot, "ms_per_step": e2e_ms,
+                "what": "lbm_init_fields (pinned host rho,u,T) + lbm_step(1) + lbm_get_macroscopic (pinned host), every step"},
+        "gpu_launches": launches * K,
+        "clocks": clocks,
+        "wall_s_timed_region": wall, "build_s": t_build,
+    }
+    if args.cpu_baseline_seconds > 0 and world >= 1:
+        o = oracle_grid(case)
+        v, nf, nu, dt = oracle_rate(o, args.cpu_baseline_seconds)
+        line["cpu_baseline"] = {"value": v, "unit": "MLUPS", "cores": 1, "kind": "oracle", "host_cores": os.cpu_count(),
+                                "sample": "%d fine steps of the schedule on the full grid (%d cell updates, %.1f s)" % (nf, nu, dt)}
+    print(json.dumps(line), flush=True)
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -223,8 +223,14 @@ class Grid:
     def kernel_name(self):
         return lib().lbm_kernel_name(self.h).decode()
 
-    def macroscopic(self):
-        r = np.zeros(self.ntot); u = np.zeros(self.ntot); v = np.zeros(self.ntot); T = np.zeros(self.ntot)
+    def macroscopic(self, out=None):
+        """rho, ux, uy, T of every stored cell; `out` = four caller-owned float64 arrays (e.g. pinned) to fill."""
+        if out is not None:
+            r, u, v, T = out
+            for x in out:
+                assert x.dtype == np.float64 and x.size == self.ntot and x.flags.c_contiguous
+        else:
+            r = np.zeros(self.ntot); u = np.zeros(self.ntot); v = np.zeros(self.ntot); T = np.zeros(self.ntot)
         _check("lbm_get_macroscopic", lib().lbm_get_macroscopic(self.h, _ptr(r), _ptr(u), _ptr(v), _ptr(T)))
         return r, u, v, T
 

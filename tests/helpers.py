@@ -37,3 +37,31 @@ def conserved_sums(g, Q_cx=None, Q_cy=None):
             e += g.populations(l, 1)[keep].sum()
         E += a * e
     return np.array([M, PX, PY, E])
+
+
+def gpu_from_case(case, precision=64, init=True):
+    """CUDA-path simulation of the same Case through the C ABI (tests marked gpu)."""
+    from paper_2504_04465_b200 import lbm
+    g = lbm.Grid.from_case(case, precision=precision)
+    g.bind()
+    if init:
+        cells = [g.cells(l)[:2] for l in range(g.depth + 1)]
+        rho, ux, uy, T = W.eval_fields(case, cells)
+        rc = g.init_fields(rho, ux, uy, T)
+        assert rc == 0, "lbm_init_fields status %d" % rc
+    return g
+
+
+def max_pop_diff(g, o, which=(0,)):
+    """max over levels, cells and components of |S_gpu - S_oracle| (ghost cells included)."""
+    d = 0.0
+    for l in range(o.depth + 1):
+        if o.n[l] == 0:
+            continue
+        for w in which:
+            d = max(d, float(np.abs(g.populations(l, w) - o.populations(l, w)).max()))
+    return d
+
+
+def rel_linf(a, b):
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))

@@ -1,0 +1,115 @@
+"""CPU checks of the boundary: the C-ABI library loads, exports every symbol include/lbm.h declares, and its
+host grid builder (row a11 of SURVEY.md Sec. 8(a)) agrees BIT FOR BIT with the oracle's independent builder:
+cells, types, neighbour lists, ghost lists, unknown masks and the level schedule (north_star: "neighbor lists
+and level schedules must be bit-exact").  No compute call is made (there is no GPU here)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2504_04465_b200 import lbm, workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "lbm.h")).read()
+    declared = sorted(set(re.findall(r"\b(lbm_[a-z_0-9]+)\s*\(", hdr)))
+    assert sorted(lbm.SYMBOLS) == declared
+    L = lbm.lib()
+    for s in declared:
+        assert hasattr(L, s), s
+
+
+def test_struct_layout_matches_header():
+    # the ctypes mirror of lbm_config / lbm_grid_info has the size the C compiler gives the header's structs
+    import subprocess
+    import tempfile
+    src = '#include <stdio.h>\n#include "lbm.h"\nint main(){printf("%zu %zu\\n", sizeof(lbm_config), sizeof(lbm_grid_info));return 0;}\n'
+    with tempfile.TemporaryDirectory() as d:
+        p = os.path.join(d, "s.c")
+        open(p, "w").write(src)
+        subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), p, "-o", os.path.join(d, "s")])
+        a, b = map(int, subprocess.check_output([os.path.join(d, "s")]).split())
+    assert a == C.sizeof(lbm.LbmConfig)
+    assert b == C.sizeof(lbm.LbmGridInfo)
+
+
+CASES = {
+    "tgv64": lambda: W.tgv(64),
+    "cavity": lambda: W.cavity(),
+    "cavity_q13": lambda: W.cavity(scale=0.5, lattice=13),
+    "cylinder_small": lambda: W.cylinder(D=40, depth=3, radii=(3, 5, 8)),
+    "riemann_neumann": lambda: W.riemann(n=64),
+    "riemann_periodic": lambda: W.riemann(n=48, periodic=True),
+    "naca_small": lambda: W.naca(chord=64, depth=3, radii=(1, 2.5, 5), aoa_deg=4.0),
+    "naca_supersonic": lambda: W.naca(chord=64, depth=2, radii=(1, 2.5), mach=1.5),
+    "patch_q21": lambda: W.patch(lattice=21),
+    "patch_depth2": lambda: W.patch(nc=48, lo=8, hi=40, depth=2),
+    "stripe_q37": lambda: W.stripe(lattice=37),
+    "walled_patch": lambda: W.patch(periodic=False),
+}
+
+
+@pytest.mark.parametrize("name", sorted(CASES))
+def test_host_builder_bit_exact_against_oracle_builder(name):
+    case = CASES[name]()
+    g = lbm.Grid.from_case(case)
+    o = O.OracleGrid(O.make_config(**case.model_kwargs()), case.mesh.split, case.mesh.solid)
+    assert g.n == o.n
+    for l in range(g.depth + 1):
+        for a, b in zip(g.cells(l), o.cells(l)):
+            assert np.array_equal(a, b)
+        assert np.array_equal(g.nbr(l), o.nbr(l))
+        assert g.tau(l) == o.tau(l)
+        if l >= 1:
+            for a, b in zip(g.ghosts(l), o.ghosts(l)):
+                assert np.array_equal(a, b)
+    for a, b in zip(g.schedule(), o.schedule()):
+        assert np.array_equal(a, b)
+    info = g.info
+    assert info.updates_per_coarse_step == sum(g.n[l] << (g.depth - l) for l in range(g.depth + 1))
+    g.close()
+
+
+def test_invalid_arguments_are_rejected():
+    with pytest.raises(lbm.LbmError) as e:
+        lbm.Grid(lbm.make_config(lattice=10, nx_coarse=8, ny_coarse=8))
+    assert e.value.code == lbm.EINVAL
+    with pytest.raises(lbm.LbmError) as e:
+        lbm.Grid(lbm.make_config(lattice=9, collision=lbm.RR, ddf=1, nx_coarse=8, ny_coarse=8))
+    assert e.value.code == lbm.EINVAL
+    with pytest.raises(lbm.LbmError) as e:
+        lbm.Grid(lbm.make_config(lattice=9, tau0=0.4, nx_coarse=8, ny_coarse=8))
+    assert e.value.code == lbm.EINVAL
+    # a level-1 cell split although its level-2 parent is not: not a quadtree
+    cfg = lbm.make_config(lattice=9, depth=2, nx_coarse=8, ny_coarse=8)
+    with pytest.raises(lbm.LbmError) as e:
+        lbm.Grid(cfg, split=[None, np.array([[4, 4]], np.int32), None])
+    assert e.value.code == lbm.EMESH
+    # two interfaces with no room for the ghost band between them (every child of the level-2 patch split again)
+    s2 = np.array([[x, y] for x in range(2, 6) for y in range(2, 6)], np.int32)
+    s1 = np.array([[x, y] for x in range(4, 12) for y in range(4, 12)], np.int32)
+    with pytest.raises(lbm.LbmError) as e:
+        lbm.Grid(cfg, split=[None, s1, s2])
+    assert e.value.code == lbm.EMESH
+    with pytest.raises(RuntimeError):
+        O.OracleGrid(O.make_config(lattice=9, depth=2, nx_coarse=8, ny_coarse=8), [None, s1, s2])
+
+
+def test_compute_calls_fail_loudly_without_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    g = lbm.Grid.from_case(W.tgv(16))
+    with pytest.raises(lbm.LbmError) as e:
+        g.bind()
+    assert e.value.code == lbm.ECUDA
+    z = np.zeros(g.ntot)
+    assert g.init_fields(z + 1, z, z) == lbm.ESTATE      # not bound: no silent CPU path
+    with pytest.raises(lbm.LbmError):
+        g.step(1)
+    g.close()

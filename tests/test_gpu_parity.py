@@ -1,0 +1,210 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are north_star's: max|df| <= 1e-12 (fp64) / 1e-5 (fp32) after one step, rho and u
+relative L-inf <= 1e-9 (fp64) / 1e-4 (fp32) after 1000 steps on the laminar configs.  Sizes span several
+128-thread tiles and a ragged tail; ghost cells of both kinds are compared too."""
+import numpy as np
+import pytest
+
+from paper_2504_04465_b200 import workloads as W
+from helpers import gpu_from_case, max_pop_diff, oracle_from_case, rel_linf
+
+pytestmark = pytest.mark.gpu
+
+TOL_F = {64: 1e-12, 32: 1e-5}
+TOL_M = {64: 1e-9, 32: 1e-4}
+
+
+def which_of(case):
+    w = [0]
+    if case.ddf:
+        w.append(1)
+    return tuple(w)
+
+
+def check_macro(g, o, tol, T=False):
+    gm, om = g.macroscopic(), o.macroscopic()
+    assert rel_linf(gm[0], om[0]) <= tol
+    uref = max(np.abs(om[1]).max(), np.abs(om[2]).max(), 1e-300)
+    assert np.abs(gm[1] - om[1]).max() / uref <= tol
+    assert np.abs(gm[2] - om[2]).max() / uref <= tol
+    if T:
+        assert rel_linf(gm[3], om[3]) <= tol
+
+
+def run_pair(case, precision, ncoarse):
+    g = gpu_from_case(case, precision)
+    o = oracle_from_case(case)
+    d0 = max_pop_diff(g, o, which_of(case))          # initialisation + iteration-0 coupling
+    g.step(ncoarse)
+    assert g.sync() == 0
+    assert o.step(ncoarse) == 0
+    return g, o, d0
+
+
+# ------------------------------------------------------------------ config 1: Taylor-Green, D2Q9 BGK
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("collision", [W.BGK, W.RR])
+def test_config1_tgv(precision, collision):
+    case = W.tgv(64, collision=collision)
+    g, o, d0 = run_pair(case, precision, 1)
+    assert d0 <= TOL_F[precision]
+    assert max_pop_diff(g, o) <= TOL_F[precision]
+    g.step(99); o.step(99)
+    assert g.sync() == 0
+    check_macro(g, o, TOL_M[precision])
+    if precision == 64:
+        # physics: amplitude decay exp(-2 nu k^2 t) within the O(k^2) lattice error (pin P6, here on the GPU)
+        m = case.meta
+        u = g.macroscopic()[1]
+        assert abs(np.abs(u).max() / m["u0"] - np.exp(-2 * m["nu"] * m["k"] ** 2 * 100)) < 2e-3
+    g.close()
+
+
+@pytest.mark.parametrize("n", [1, 5, 37, 130])
+def test_ragged_sizes_uniform_periodic(n):
+    # n*n is not a multiple of the 128-thread tile (n = 1: every link points to the cell itself)
+    case = W.tgv(n, u0=0.03)
+    g, o, d0 = run_pair(case, 64, 3)
+    assert max_pop_diff(g, o) <= 1e-12
+    g.close()
+
+
+# ------------------------------------------------------------------ config 2: cavity, 2 levels, RR
+@pytest.mark.parametrize("precision", [64, 32])
+def test_config2_cavity_one_coarse_step(precision):
+    case = W.cavity()
+    g, o, d0 = run_pair(case, precision, 1)
+    assert d0 <= TOL_F[precision]
+    assert max_pop_diff(g, o) <= TOL_F[precision]
+    g.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_config2_cavity_1000_fine_steps(precision):
+    case = W.cavity()
+    g, o, _ = run_pair(case, precision, 500)
+    check_macro(g, o, TOL_M[precision])
+    if precision == 64:
+        assert max_pop_diff(g, o) <= 1e-10
+    g.close()
+
+
+def test_config2_cavity_trace_eq_and_bgk():
+    for kw in (dict(trace_eq=1), dict(collision=W.BGK)):
+        case = W.cavity(scale=0.5, **kw)
+        g, o, _ = run_pair(case, 64, 2)
+        assert max_pop_diff(g, o) <= 1e-12
+        g.close()
+
+
+# ------------------------------------------------------------------ config 3: cylinder, graded levels
+@pytest.mark.parametrize("precision", [64, 32])
+def test_config3_cylinder_scaled(precision):
+    case = W.cylinder(D=40, depth=3, radii=(3, 5, 8))
+    g, o, d0 = run_pair(case, precision, 1)
+    assert d0 <= TOL_F[precision]
+    assert max_pop_diff(g, o) <= TOL_F[precision]
+    g.step(3); o.step(3)
+    assert g.sync() == 0
+    check_macro(g, o, TOL_M[precision])
+    g.close()
+
+
+# ------------------------------------------------------------------ config 4: D2Q37 polynomial + g + sensor
+@pytest.mark.parametrize("periodic", [False, True])
+def test_config4_riemann_scaled(periodic):
+    case = W.riemann(n=96, periodic=periodic)
+    g, o, d0 = run_pair(case, 64, 1)
+    assert d0 <= 1e-12
+    assert max_pop_diff(g, o, (0, 1)) <= 1e-12
+    g.step(4); o.step(4)
+    assert g.sync() == 0
+    check_macro(g, o, 1e-9, T=True)
+    g.close()
+
+
+# ------------------------------------------------------------------ config 5: D2Q21 numerical eq. + g + sensor
+@pytest.mark.parametrize("mach,aoa", [(0.8, 0.0), (1.5, 4.0)])
+def test_config5_naca_scaled(mach, aoa):
+    case = W.naca(chord=64, depth=3, radii=(1, 2.5, 5), mach=mach, aoa_deg=aoa)
+    g, o, d0 = run_pair(case, 64, 1)
+    assert d0 <= 1e-12
+    assert max_pop_diff(g, o, (0, 1)) <= 1e-12
+    assert max_pop_diff(g, o, (2,)) <= 1e-9       # multipliers: conditioned by the Jacobian, not by f
+    check_macro(g, o, 1e-9, T=True)
+    g.close()
+
+
+# ------------------------------------------------------------------ the other lattices / model combinations
+def smooth_fields(nc, depth, cs2, thermal=False):
+    L = nc << depth
+    k = 2 * np.pi / L
+
+    def fields(level, ix, iy):
+        x, y = W.centres(level, ix, iy)
+        rho = 1.0 + 0.05 * np.sin(k * x) * np.cos(2 * k * y)
+        ux = 0.08 * np.sin(k * y + 0.3) + 0.02
+        uy = -0.05 * np.cos(k * x) + 0.01
+        T = cs2 * (1.0 + (0.06 * np.cos(k * x + k * y) if thermal else 0.0))
+        return rho, ux, uy, T
+    return fields
+
+
+@pytest.mark.parametrize("lattice", [13, 21, 37])
+@pytest.mark.parametrize("collision", [W.BGK, W.RR])
+def test_high_order_lattices_patch(lattice, collision):
+    nc = 48
+    case = W.patch(nc=nc, lo=12, hi=36, lattice=lattice, collision=collision, tau0=0.7,
+                   fields=smooth_fields(nc, 1, W.CS2[lattice]))
+    g, o, d0 = run_pair(case, 64, 2)
+    assert d0 <= 1e-12
+    assert max_pop_diff(g, o) <= 1e-12
+    g.close()
+
+
+@pytest.mark.parametrize("lattice", [21, 37])
+def test_numerical_equilibrium_ddf_sensor_stripe(lattice):
+    nc = 48
+    T0 = 0.65 if lattice == 21 else 0.4
+    case = W.stripe(nc=nc, lo=12, hi=36, lattice=lattice, collision=W.NUMEQ, ddf=1, sensor=1, tau0=0.6, T0=T0,
+                    sensor_A=1.35, fields=smooth_fields(nc, 1, T0, thermal=True))
+    g, o, d0 = run_pair(case, 64, 2)
+    assert d0 <= 1e-12
+    assert max_pop_diff(g, o, (0, 1)) <= 1e-12
+    g.close()
+
+
+def test_multilevel_depth2_patch_fp64():
+    nc = 48
+    case = W.patch(nc=nc, lo=8, hi=40, depth=2, collision=W.RR, tau0=0.6, fields=smooth_fields(nc, 2, 1.0 / 3.0))
+    g, o, d0 = run_pair(case, 64, 3)
+    assert max_pop_diff(g, o) <= 1e-12
+    g.close()
+
+
+def test_step_zero_and_repeated_init():
+    case = W.tgv(32)
+    g, o, _ = run_pair(case, 64, 0)
+    assert max_pop_diff(g, o) == 0.0 or max_pop_diff(g, o) <= 1e-15
+    g.step(5); o.step(5)
+    # re-initialising restarts the run
+    cells = [g.cells(0)[:2]]
+    rho, ux, uy, T = W.eval_fields(case, cells)
+    assert g.init_fields(rho, ux, uy, T) == 0
+    assert o.init_fields(rho, ux, uy, T) == 0
+    g.step(1); o.step(1)
+    assert g.sync() == 0
+    assert max_pop_diff(g, o) <= 1e-12
+    g.close()
+
+
+def test_unstable_state_is_reported():
+    from paper_2504_04465_b200 import lbm
+    case = W.tgv(16)
+    g = gpu_from_case(case)
+    f = g.populations(0, 0)
+    f[3, :] = -1.0      # negative density in one cell
+    g.set_populations(0, 0, f)
+    g.step(1)
+    assert g.sync() == lbm.EUNSTABLE
+    g.close()
