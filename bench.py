@@ -39,20 +39,20 @@ FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only 
 def make_case(name, scale):
     if name == "cylinder":
         D = int(round(200 * scale))
-        return W.cylinder(D=D), dict(workload="cylinder (BASELINE configs[2]): D2Q9-RR, D=%d, 64Dx64D, 6 levels" % D, steps=20)
+        return W.cylinder(D=D), dict(workload="cylinder (BASELINE configs[2]): D2Q9-RR, D=%d, 64Dx64D, 6 levels" % D, steps=300)
     if name == "uniform":
         n = int(round(4096 * scale))
-        return W.tgv(n), dict(workload="uniform periodic %dx%d tree-stored D2Q9-BGK Taylor-Green (configs[0] scaled)" % (n, n), steps=200)
+        return W.tgv(n), dict(workload="uniform periodic %dx%d tree-stored D2Q9-BGK Taylor-Green (configs[0] scaled)" % (n, n), steps=4000)
     if name == "cavity":
-        return W.cavity(scale), dict(workload="cavity (BASELINE configs[1]): D2Q9-RR, 2 levels, coarse %d^2" % int(128 * scale), steps=2000)
+        return W.cavity(scale), dict(workload="cavity (BASELINE configs[1]): D2Q9-RR, 2 levels, coarse %d^2" % int(128 * scale), steps=100000)
     if name == "cavity8":
-        return W.cavity(8 * scale), dict(workload="cavity x8: D2Q9-RR, 2 levels, coarse %d^2" % int(1024 * scale), steps=200)
+        return W.cavity(8 * scale), dict(workload="cavity x8: D2Q9-RR, 2 levels, coarse %d^2" % int(1024 * scale), steps=10000)
     if name == "riemann":
         n = int(round(2048 * scale))
-        return W.riemann(n=n), dict(workload="riemann (BASELINE configs[3]): D2Q37 polynomial+g+sensor, %d^2, Neumann box" % n, steps=50)
+        return W.riemann(n=n), dict(workload="riemann (BASELINE configs[3]): D2Q37 polynomial+g+sensor, %d^2, Neumann box" % n, steps=200)
     if name == "naca":
         c = int(round(1024 * scale))
-        return W.naca(chord=c), dict(workload="naca (BASELINE configs[4]): D2Q21 numerical eq.+g+sensor, chord %d, 7 levels" % c, steps=3)
+        return W.naca(chord=c), dict(workload="naca (BASELINE configs[4]): D2Q21 numerical eq.+g+sensor, chord %d, 7 levels" % c, steps=8)
     raise SystemExit("unknown workload %r" % name)
 
 
@@ -170,6 +170,23 @@ def run_reference(args, case, info):
     print(json.dumps(line), flush=True)
 
 
+# ----------------------------------------------------------------------------- N > 1: replicas, max-over-ranks timing
+def reduce_max_over_ranks(values, world, device="cpu"):
+    """The slowest rank defines the job time (contract: time = max over ranks).  Works on any backend (nccl on the
+    GPU box, gloo in tests/test_bench_host.py)."""
+    import torch
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def aggregate_mlups(updates_per_rank_step, steps, world, ms):
+    """Whole-job throughput of `world` independent replicas (weak scaling): all ranks' updates / the slowest rank's time."""
+    return updates_per_rank_step * steps * world / (ms * 1e-3) / 1e6
+
+
 # ----------------------------------------------------------------------------- CUDA arm
 def main():
     ap = argparse.ArgumentParser()
@@ -255,27 +272,26 @@ def main():
                 e2e_ms += ev0.elapsed_time(ev1)
     e2e_ms /= max(args.e2e_steps, 1)
 
-    t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = float(t[0]), float(t[1])
+    ms, e2e_ms = reduce_max_over_ranks([ms, e2e_ms], world, dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     K = args.steps
-    total_upd = upd * K * world
-    mlups = total_upd / (ms * 1e-3) / 1e6
+    mlups = aggregate_mlups(upd, K, world, ms)
     bpu = algorithmic_bytes_per_update(case, args.precision)
     peaks, peak_src = measured_peaks()
     peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
     achieved = upd * K * bpu / (ms * 1e-3) / 1e9          # this rank's kernel: all launches of the region are the sweep kernel
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")   # dram bytes per cell update from the committed ncu capture
-    if os.path.exists(tp):
+    # dram bytes per launch of the dominant kernel (finest level's sweep) from the committed ncu --set full capture
+    traffic = traffic_src = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp) and args.scale == 1.0:
         try:
-            traffic = json.load(open(tp)).get("%s_f%d" % (args.workload, args.precision))
+            e = json.load(open(tp)).get("%s_f%d" % (args.workload, args.precision))
+            if e and int(e["cells_per_launch"]) == int(g.n[0]):
+                traffic, traffic_src = e["bytes_per_launch"], e["source"]
         except Exception:
             traffic = None
     n_all = ntot
@@ -292,7 +308,10 @@ def main():
         "mlups": {"actual": mlups, "paper_eq13": n_all * (1 << depth) * K * world / (ms * 1e-3) / 1e6,
                   "fine_equivalent": fine_equivalent_cells(case) * (1 << depth) * K * world / (ms * 1e-3) / 1e6},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "peak_source": peak_src, "bytes_per_update": bpu,
+                     "traffic": traffic, "traffic_source": traffic_src,
+                     "algorithmic_bytes_per_launch": int(g.n[0]) * bpu, "kernel": "%s, finest level (%d cells per launch)" % (g.kernel_name(), g.n[0]),
+                     "achieved_is": "algorithmic bytes of all level sweeps of the timed region / its CUDA-event time (every launch is this kernel)",
+                     "peak_source": peak_src, "bytes_per_update": bpu,
                      "frac_of_nominal_8TBs": achieved / 8000.0},
         "e2e": {"value": upd * world / (e2e_ms * 1e-3) / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 4 * 8 * ntot,
                 "d2h_bytes_per_step": 4 * 8 * ntot, "ms_per_step": e2e_ms,
