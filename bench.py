@@ -244,6 +244,14 @@ def main():
     # ---- device-resident throughput: W warm-up steps, then exactly K steps between CUDA events on the bound stream
     g.step(args.warmup)
     assert g.sync() == 0
+    # burst figure (GPU still cool, ~30 ms region: comparable with MEASURED_PEAKS' best-of-10 copy); the headline
+    # `value` below is the sustained figure over the full K steps, which on these 1 kW parts runs under sw_power_cap
+    g.step(3)
+    est = max(g.last_step_ms() / 3, 1e-4)
+    kb = int(min(max(3, 30.0 / est), max(3, args.steps)))
+    g.step(kb)
+    burst_ms = g.last_step_ms() / kb
+    assert g.sync() == 0
     barrier()
     clk = ClockSampler(local)
     t0 = time.perf_counter()
@@ -313,6 +321,9 @@ def main():
                      "achieved_is": "algorithmic bytes of all level sweeps of the timed region / its CUDA-event time (every launch is this kernel)",
                      "peak_source": peak_src, "bytes_per_update": bpu,
                      "frac_of_nominal_8TBs": achieved / 8000.0},
+        "burst": {"steps": kb, "ms_per_step": burst_ms, "value": upd / (burst_ms * 1e-3) / 1e6, "unit": "MLUPS (this rank)",
+                  "roofline_frac": upd * bpu / (burst_ms * 1e-3) / 1e9 / peak,
+                  "what": "short region right after warm-up, before the power cap settles; `value` is the sustained figure"},
         "e2e": {"value": upd * world / (e2e_ms * 1e-3) / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 4 * 8 * ntot,
                 "d2h_bytes_per_step": 4 * 8 * ntot, "ms_per_step": e2e_ms,
                 "what": "lbm_init_fields (pinned host rho,u,T) + lbm_step(1) + lbm_get_macroscopic (pinned host), every step"},

@@ -151,6 +151,15 @@ double lbm_last_step_ms(lbm_grid* g);
 /* Name of the compiled sweep kernel this grid dispatches to (static string), for profiles. */
 const char* lbm_kernel_name(const lbm_grid* g);
 
+
+/* Measured FMA peak of the current device's plain fp64 (precision 64) or fp32 (32) pipe, in TFLOP/s (2 flop per
+ * FMA): 8 independent dependent-FMA chains per thread, every SM filled to its thread limit, launches repeated for
+ * about `seconds` of device time, best launch reported.  This is the denominator of the "alu" rooflines of the
+ * D2Q37 and numerical-equilibrium paths (north_star: "FP64/FP32 pipe utilisation against peak").
+ * tflops: HOST out.  lanes_mhz_per_sm (HOST out, may be NULL) = FMA/s per SM / 1e6 (= lanes x clock in MHz).
+ * Uses the current device and the legacy default stream; allocates and frees one word.  LBM_ECUDA without a device. */
+int lbm_measure_fma_peak(int precision, double seconds, double* tflops, double* lanes_mhz_per_sm);
+
 #ifdef __cplusplus
 }
 #endif

@@ -17,7 +17,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liblbm_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
-CU = ["lbm_api.cu", "sweep_q9.cu", "sweep_q13.cu", "sweep_q21.cu", "sweep_q37.cu"]
+CU = ["lbm_api.cu", "peak.cu", "sweep_q9.cu", "sweep_q13.cu", "sweep_q21.cu", "sweep_q37.cu"]
 CPP = ["grid_builder.cpp"]
 HEADERS = [os.path.join(CSRC, h) for h in ("grid.hpp", "lattice.cuh", "collide.cuh", "sweep.cuh")] + [os.path.join(INCLUDE, "lbm.h")]
 

@@ -5,6 +5,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -61,6 +62,7 @@ struct lbm_grid {
   int64_t n_total = 0, launches_per_coarse = 0, updates_per_coarse = 0;
   size_t arena_bytes = 0, off_status = 0, off_scratch = 0, scratch_doubles = 0;
   bool bound = false, inited = false, own_stream = false;
+  bool pdl = true;                                // programmatic dependent launch between level sweeps (LBM_NO_PDL=1 disables)
   char* arena = nullptr;
   cudaStream_t stream = nullptr;
   int* d_status = nullptr;
@@ -97,11 +99,24 @@ const KernelSet* find_kernel_set(const lbm_config& c) {
   return nullptr;
 }
 
-int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s) {
+// n work items, `per_thread` of them per thread.  pdl: chain to the previous kernel of the stream with a programmatic
+// dependent-launch edge (only for kernels that call griddepcontrol.wait before touching mutable data: the sweep).
+int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s, int per_thread = 1, bool pdl = false) {
   if (n <= 0) return LBM_OK;
   void* args[2] = {a0, a1};
-  const unsigned grid = (unsigned)((n + BLOCK - 1) / BLOCK);
-  CK(cudaLaunchKernel(fn, dim3(grid), dim3(BLOCK), args, 0, s));
+  const int64_t threads = (n + per_thread - 1) / per_thread;
+  const unsigned grid = (unsigned)((threads + BLOCK - 1) / BLOCK);
+  if (!pdl) {
+    CK(cudaLaunchKernel(fn, dim3(grid), dim3(BLOCK), args, 0, s));
+    return LBM_OK;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  CK(cudaLaunchKernelExC(&cfg, fn, args));
   return LBM_OK;
 }
 
@@ -116,7 +131,7 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   a.fps = l > 0 ? g->dl[l - 1].ps : 0;
   a.tau = g->hg.lv[l].tau;
   a.status = g->d_status;
-  int rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream);
+  int rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream, g->ks->cells_per_thread, g->pdl);
   cur[l] ^= 1;
   return rc;
 }
@@ -358,6 +373,7 @@ int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream
   CK(cudaEventCreate(&g->ev0));
   CK(cudaEventCreate(&g->ev1));
   g->bound = true;
+  if (const char* e = getenv("LBM_NO_PDL")) g->pdl = !(e[0] == '1');
   // graphs: one coarse step from either parity of the coarsest level, and K steps for launch-bound grids
   for (int p = 0; p < 2; ++p) {
     int rc = capture(g, p, 1, &g->g1[p]);

@@ -44,195 +44,244 @@ struct PopLayout {
   static constexpr int NPOP = L0 + (COLL == LBM_NUMEQ ? NLAMBDA : 0);
 };
 
+// Cells per thread: the fp32 weakly compressible kernels keep two consecutive Morton cells per thread (64-bit list
+// loads and 64-bit stores, twice the gathers in flight per warp: with 4-byte populations one cell per thread leaves
+// the memory system short of outstanding bytes, profiles/r01_ncu_uniform_f32.md); everything else one cell.
+template <int Q, typename T, int COLL, bool DDF>
+constexpr int cells_per_thread = (sizeof(T) == 4 && !DDF && COLL != LBM_NUMEQ && Q <= 13) ? 2 : 1;
+
+// Resident CTAs per SM asked of ptxas (register cap): D2Q9 runs at 8 x 128 threads (64 registers).
+template <int Q, typename T, int COLL, bool DDF>
+constexpr int min_ctas_per_sm = (Q == 9 && !DDF && COLL != LBM_NUMEQ) ? 8 : 1;
+
+template <typename T, int N> struct alignas(sizeof(T) * N) Vec { T v[N]; };
+
+// Programmatic dependent launch (sm_90+): consecutive level sweeps of the schedule are chained with programmatic
+// edges, so the next sweep's CTAs become resident while this sweep drains and load their static tables (type, list,
+// ghost rows) before waiting for this sweep's memory to be visible.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
-__global__ void __launch_bounds__(128) sweep_kernel(const LevelArgs a, const ModelParams p) {
+__global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep_kernel(const LevelArgs a, const ModelParams p) {
   using PL = PopLayout<Q, DDF, COLL>;
   constexpr bool NUMEQ = COLL == LBM_NUMEQ;
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= a.n) return;
-  const int tb = a.type[c];
-  const int type = tb & TYPE_MASK;
+  constexpr int CPT = cells_per_thread<Q, T, COLL, DDF>;
+  pdl_launch_dependents();
+  const int c0 = (blockIdx.x * blockDim.x + threadIdx.x) * CPT;
+  if (c0 >= a.n) return;
   const T* __restrict__ So = (const T*)a.So;
   T* __restrict__ Sn = (T*)a.Sn;
   const long long ps = a.ps;
-  T f[Q], g[Q], lam[NLAMBDA];
 
-  if (type == LBM_DIRICHLET) {
-    // equilibrium Dirichlet cell: imposed (rho,u,T); rho optionally from the nearest interior cell
-    const int side = tb >> TYPE_SIDE_SHIFT;
-    T rho = T(p.bc_rho[side]);
-    if (p.bc_kind[side] == LBM_BC_DIRICHLET_EQ_RHO_EXTRAP) {
-      const int s = a.aux[c];
-      rho = T(0);
+  // ---- static tables (never written after lbm_grid_bind): cell types, links, boundary sources.  Planes are padded to
+  // a multiple of 64 cells, so the vector accesses of a ragged last thread stay inside the arrays; a cell index >= n is
+  // handled as a link-less fine ghost (it moves padding to padding).
+  int type[CPT], side[CPT], self[CPT], nb[CPT][Q];
+  {
+    const Vec<unsigned char, CPT> tv = *reinterpret_cast<const Vec<unsigned char, CPT>*>(a.type + c0);
 #pragma unroll
-      for (int i = 0; i < Q; ++i) rho += So[i * ps + s];
+    for (int j = 0; j < CPT; ++j) {
+      const bool valid = c0 + j < a.n;
+      type[j] = valid ? (tv.v[j] & TYPE_MASK) : LBM_FINE_GHOST;
+      side[j] = tv.v[j] >> TYPE_SIDE_SHIFT;
     }
-    const T Tb = (NUMEQ || DDF) ? T(p.bc_T[side]) : T(cs2_v<Q>);
-    if constexpr (NUMEQ) {
+    static_for<1, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      const Vec<int, CPT> nv = *reinterpret_cast<const Vec<int, CPT>*>(a.nbr + (long long)(I - 1) * ps + c0);
 #pragma unroll
-      for (int k = 0; k < NLAMBDA; ++k) lam[k] = So[(PL::L0 + k) * ps + c];
-    }
-    const int it = equilibrium<Q, T, COLL, DDF>(p, rho, T(p.bc_ux[side]), T(p.bc_uy[side]), Tb, lam, f, g);
+      for (int j = 0; j < CPT; ++j) nb[j][I] = (c0 + j < a.n) ? nv.v[j] : LBM_LINK_NONE;
+    });
 #pragma unroll
-    for (int i = 0; i < Q; ++i) Sn[i * ps + c] = f[i];
-    if constexpr (DDF) {
-#pragma unroll
-      for (int i = 0; i < Q; ++i) Sn[(PL::G0 + i) * ps + c] = g[i];
-    }
-    if constexpr (NUMEQ) {
-#pragma unroll
-      for (int k = 0; k < NLAMBDA; ++k) Sn[(PL::L0 + k) * ps + c] = lam[k];
-    }
-    if (it < 0) atomicOr(a.status, FLAG_NEWTON);
-    if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
-    return;
-  }
-
-  // a NEUMANN cell replicates the complete update of its source cell (reading S13)
-  const int self = (type == LBM_NEUMANN) ? a.aux[c] : c;
-
-  // ---- step 1: gather (pull form of Eq. 31).  Links first (coalesced, independent loads) ...
-  int nb[Q];
-  nb[0] = self;
-  bool special = false;     // any velocity-bounce-back or (coarse ghost) unknown link
-  static_for<1, Q>([&](auto ic) {
-    constexpr int I = decltype(ic)::value;
-    nb[I] = a.nbr[(long long)(I - 1) * ps + c];
-    special |= (nb[I] <= LBM_LINK_VBB0) || (nb[I] == LBM_LINK_NONE);
-  });
-  // ... then the populations, branch-free: a wall link reads the cell's own opposite population
-  // (half-way bounce-back), a NONE link the cell's own value (fine ghosts, S6; fixed up below
-  // for coarse ghosts), any other link the neighbour's.
-  static_for<0, Q>([&](auto ic) {
-    constexpr int I = decltype(ic)::value;
-    constexpr int O = Lat<Q>::t.opp[I];
-    const int n = nb[I];
-    const int src = n >= 0 ? n : self;
-    const int comp = (n >= 0 || n == LBM_LINK_NONE) ? I : O;
-    f[I] = So[comp * ps + src];
-    if constexpr (DDF) g[I] = So[(PL::G0 + comp) * ps + src];
-  });
-
-  if (special) {
-    if (type == LBM_COARSE_GHOST) {
-      // coalescence (Eq. 4): unknown directions only, mean over the children that exist
-      const int* ch = a.g_child + 4ll * a.aux[c];
-      const int c0 = ch[0], c1 = ch[1], c2 = ch[2], c3 = ch[3];
-      const T nf = T((c0 >= 0) + (c1 >= 0) + (c2 >= 0) + (c3 >= 0));
-      const T* F = (const T*)a.fine;
-      const long long fps = a.fps;
-      static_for<1, Q>([&](auto ic) {
-        constexpr int I = decltype(ic)::value;
-        if (nb[I] == LBM_LINK_NONE) {
-          T s = T(0);
-          if (c0 >= 0) s += F[I * fps + c0];
-          if (c1 >= 0) s += F[I * fps + c1];
-          if (c2 >= 0) s += F[I * fps + c2];
-          if (c3 >= 0) s += F[I * fps + c3];
-          f[I] = s / nf;
-          if constexpr (DDF) {
-            T sg = T(0);
-            if (c0 >= 0) sg += F[(PL::G0 + I) * fps + c0];
-            if (c1 >= 0) sg += F[(PL::G0 + I) * fps + c1];
-            if (c2 >= 0) sg += F[(PL::G0 + I) * fps + c2];
-            if (c3 >= 0) sg += F[(PL::G0 + I) * fps + c3];
-            g[I] = sg / nf;
-          }
-        }
-      });
-    }
-    // velocity bounce-back (Ladd): + 2 w_i rho_w (xi_i . u_w) / c_s^2, rho_w local (S11)
-    bool vbb = false;
-    static_for<1, Q>([&](auto ic) { vbb |= nb[decltype(ic)::value] <= LBM_LINK_VBB0; });
-    if (vbb) {
-      T rho_w = T(0);
-#pragma unroll
-      for (int j = 0; j < Q; ++j) rho_w += So[j * ps + self];
-      static_for<1, Q>([&](auto ic) {
-        constexpr int I = decltype(ic)::value;
-        if (nb[I] <= LBM_LINK_VBB0) {
-          const int side = LBM_LINK_VBB0 - nb[I];
-          constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
-          constexpr double w2 = 2.0 * Lat<Q>::t.w[I];
-          const T xu = T(cx) * T(p.bc_ux[side]) + T(cy) * T(p.bc_uy[side]);
-          f[I] += T(w2) * rho_w * xu / T(cs2_v<Q>);
-        }
-      });
+    for (int j = 0; j < CPT; ++j) {
+      // a NEUMANN cell replicates the complete update of its source cell (reading S13)
+      self[j] = (type[j] == LBM_NEUMANN) ? a.aux[c0 + j] : c0 + j;
+      nb[j][0] = self[j];
     }
   }
+  pdl_wait();      // from here on: data written by the previous sweeps of the stream
 
-  if (type == LBM_FINE_GHOST) {
-    // fine ghost cells stream without colliding; lambda stays
+  // ---- step 1: gather (pull form of Eq. 31), branch-free: a wall link reads the cell's own opposite population
+  // (half-way bounce-back), a NONE link the cell's own value (fine ghosts, S6; fixed up below for coarse
+  // ghosts), any other link the neighbour's.
+  T f[CPT][Q], g[CPT][Q], lam[CPT][NLAMBDA];
 #pragma unroll
-    for (int i = 0; i < Q; ++i) Sn[i * ps + c] = f[i];
-    if constexpr (DDF) {
-#pragma unroll
-      for (int i = 0; i < Q; ++i) Sn[(PL::G0 + i) * ps + c] = g[i];
-    }
-    if constexpr (NUMEQ) {
-#pragma unroll
-      for (int k = 0; k < NLAMBDA; ++k) Sn[(PL::L0 + k) * ps + c] = So[(PL::L0 + k) * ps + c];
-    }
-    return;
+  for (int j = 0; j < CPT; ++j) {
+    static_for<0, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      constexpr int O = Lat<Q>::t.opp[I];
+      const int n = nb[j][I];
+      const int src = n >= 0 ? n : self[j];
+      const int comp = (n >= 0 || n == LBM_LINK_NONE) ? I : O;
+      f[j][I] = So[comp * ps + src];
+      if constexpr (DDF) g[j][I] = So[(PL::G0 + comp) * ps + src];
+    });
   }
 
-  if constexpr (NUMEQ) {
-    if (type == LBM_COARSE_GHOST) {   // Eq. 6: warm start from the mean of the children's multipliers
-      const int* ch = a.g_child + 4ll * a.aux[c];
-      int nf = 0;
 #pragma unroll
-      for (int k = 0; k < NLAMBDA; ++k) lam[k] = T(0);
-      for (int j = 0; j < 4; ++j) {
-        const int cj = ch[j];
-        if (cj < 0) continue;
-        ++nf;
+  for (int j = 0; j < CPT; ++j) {
+    const int c = c0 + j;
+    if (type[j] == LBM_DIRICHLET) {
+      // equilibrium Dirichlet cell: imposed (rho,u,T); rho optionally from the nearest interior cell
+      const int sd = side[j];
+      T rho = T(p.bc_rho[sd]);
+      if (p.bc_kind[sd] == LBM_BC_DIRICHLET_EQ_RHO_EXTRAP) {
+        const int s = a.aux[c];
+        rho = T(0);
 #pragma unroll
-        for (int k = 0; k < NLAMBDA; ++k) lam[k] += ((const T*)a.fine)[(PL::L0 + k) * a.fps + cj];
+        for (int i = 0; i < Q; ++i) rho += So[i * ps + s];
       }
-#pragma unroll
-      for (int k = 0; k < NLAMBDA; ++k) lam[k] /= T(nf);
-    } else {
-#pragma unroll
-      for (int k = 0; k < NLAMBDA; ++k) lam[k] = So[(PL::L0 + k) * ps + self];
-    }
-  }
-
-  // ---- steps 2-5: moments, equilibrium, sensor, relaxation
-  T rho;
-  const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f, g, lam, rho);
-
-  // ---- store (coalesced: own slot of the new buffer)
-#pragma unroll
-  for (int i = 0; i < Q; ++i) Sn[i * ps + c] = f[i];
-  if constexpr (DDF) {
-#pragma unroll
-    for (int i = 0; i < Q; ++i) Sn[(PL::G0 + i) * ps + c] = g[i];
-  }
-  if constexpr (NUMEQ) {
-#pragma unroll
-    for (int k = 0; k < NLAMBDA; ++k) Sn[(PL::L0 + k) * ps + c] = lam[k];
-  }
-  if (it < 0) atomicOr(a.status, FLAG_NEWTON);
-  if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
-
-  if (type == LBM_COARSE_GHOST) {
-    // uniform explosion (Eq. 5, 7): every child receives the coarse post-collision state, all directions (S8)
-    const int* ch = a.g_child + 4ll * a.aux[c];
-    T* F = (T*)a.fine;
-    const long long fps = a.fps;
-    for (int j = 0; j < 4; ++j) {
-      const int cj = ch[j];
-      if (cj < 0) continue;
-#pragma unroll
-      for (int i = 0; i < Q; ++i) F[i * fps + cj] = f[i];
-      if constexpr (DDF) {
-#pragma unroll
-        for (int i = 0; i < Q; ++i) F[(PL::G0 + i) * fps + cj] = g[i];
-      }
+      const T Tb = (NUMEQ || DDF) ? T(p.bc_T[sd]) : T(cs2_v<Q>);
       if constexpr (NUMEQ) {
 #pragma unroll
-        for (int k = 0; k < NLAMBDA; ++k) F[(PL::L0 + k) * fps + cj] = lam[k];
+        for (int k = 0; k < NLAMBDA; ++k) lam[j][k] = So[(PL::L0 + k) * ps + c];
       }
+      T geq[Q];
+      const int it = equilibrium<Q, T, COLL, DDF>(p, rho, T(p.bc_ux[sd]), T(p.bc_uy[sd]), Tb, lam[j], f[j], geq);
+      if constexpr (DDF) {
+#pragma unroll
+        for (int i = 0; i < Q; ++i) g[j][i] = geq[i];
+      }
+      if (it < 0) atomicOr(a.status, FLAG_NEWTON);
+      if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+      continue;
+    }
+
+    bool special = false;     // any velocity-bounce-back or unknown link
+    static_for<1, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      special |= (nb[j][I] <= LBM_LINK_VBB0) || (nb[j][I] == LBM_LINK_NONE);
+    });
+    if (special) {
+      if (type[j] == LBM_COARSE_GHOST) {
+        // coalescence (Eq. 4): unknown directions only, mean over the children that exist
+        const int* ch = a.g_child + 4ll * a.aux[c];
+        const int k0 = ch[0], k1 = ch[1], k2 = ch[2], k3 = ch[3];
+        const T nf = T((k0 >= 0) + (k1 >= 0) + (k2 >= 0) + (k3 >= 0));
+        const T* F = (const T*)a.fine;
+        const long long fps = a.fps;
+        static_for<1, Q>([&](auto ic) {
+          constexpr int I = decltype(ic)::value;
+          if (nb[j][I] == LBM_LINK_NONE) {
+            T s = T(0);
+            if (k0 >= 0) s += F[I * fps + k0];
+            if (k1 >= 0) s += F[I * fps + k1];
+            if (k2 >= 0) s += F[I * fps + k2];
+            if (k3 >= 0) s += F[I * fps + k3];
+            f[j][I] = s / nf;
+            if constexpr (DDF) {
+              T sg = T(0);
+              if (k0 >= 0) sg += F[(PL::G0 + I) * fps + k0];
+              if (k1 >= 0) sg += F[(PL::G0 + I) * fps + k1];
+              if (k2 >= 0) sg += F[(PL::G0 + I) * fps + k2];
+              if (k3 >= 0) sg += F[(PL::G0 + I) * fps + k3];
+              g[j][I] = sg / nf;
+            }
+          }
+        });
+      }
+      // velocity bounce-back (Ladd): + 2 w_i rho_w (xi_i . u_w) / c_s^2, rho_w local (S11)
+      bool vbb = false;
+      static_for<1, Q>([&](auto ic) { vbb |= nb[j][decltype(ic)::value] <= LBM_LINK_VBB0; });
+      if (vbb) {
+        T rho_w = T(0);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) rho_w += So[i * ps + self[j]];
+        static_for<1, Q>([&](auto ic) {
+          constexpr int I = decltype(ic)::value;
+          if (nb[j][I] <= LBM_LINK_VBB0) {
+            const int sd = LBM_LINK_VBB0 - nb[j][I];
+            constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
+            constexpr double w2 = 2.0 * Lat<Q>::t.w[I];
+            const T xu = T(cx) * T(p.bc_ux[sd]) + T(cy) * T(p.bc_uy[sd]);
+            f[j][I] += T(w2) * rho_w * xu / T(cs2_v<Q>);
+          }
+        });
+      }
+    }
+
+    if (type[j] == LBM_FINE_GHOST) {
+      // fine ghost cells stream without colliding; lambda stays
+      if constexpr (NUMEQ) {
+#pragma unroll
+        for (int k = 0; k < NLAMBDA; ++k) lam[j][k] = So[(PL::L0 + k) * ps + c];
+      }
+      continue;
+    }
+
+    if constexpr (NUMEQ) {
+      if (type[j] == LBM_COARSE_GHOST) {   // Eq. 6: warm start from the mean of the children's multipliers
+        const int* ch = a.g_child + 4ll * a.aux[c];
+        int nf = 0;
+#pragma unroll
+        for (int k = 0; k < NLAMBDA; ++k) lam[j][k] = T(0);
+        for (int q = 0; q < 4; ++q) {
+          const int cq = ch[q];
+          if (cq < 0) continue;
+          ++nf;
+#pragma unroll
+          for (int k = 0; k < NLAMBDA; ++k) lam[j][k] += ((const T*)a.fine)[(PL::L0 + k) * a.fps + cq];
+        }
+#pragma unroll
+        for (int k = 0; k < NLAMBDA; ++k) lam[j][k] /= T(nf);
+      } else {
+#pragma unroll
+        for (int k = 0; k < NLAMBDA; ++k) lam[j][k] = So[(PL::L0 + k) * ps + self[j]];
+      }
+    }
+
+    // ---- steps 2-5: moments, equilibrium, sensor, relaxation
+    T rho;
+    const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f[j], g[j], lam[j], rho);
+    if (it < 0) atomicOr(a.status, FLAG_NEWTON);
+    if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+
+    if (type[j] == LBM_COARSE_GHOST) {
+      // uniform explosion (Eq. 5, 7): every child receives the coarse post-collision state, all directions (S8)
+      const int* ch = a.g_child + 4ll * a.aux[c];
+      T* F = (T*)a.fine;
+      const long long fps = a.fps;
+      for (int q = 0; q < 4; ++q) {
+        const int cq = ch[q];
+        if (cq < 0) continue;
+#pragma unroll
+        for (int i = 0; i < Q; ++i) F[i * fps + cq] = f[j][i];
+        if constexpr (DDF) {
+#pragma unroll
+          for (int i = 0; i < Q; ++i) F[(PL::G0 + i) * fps + cq] = g[j][i];
+        }
+        if constexpr (NUMEQ) {
+#pragma unroll
+          for (int k = 0; k < NLAMBDA; ++k) F[(PL::L0 + k) * fps + cq] = lam[j][k];
+        }
+      }
+    }
+  }
+
+  // ---- store (coalesced, CPT-wide: own slots of the new buffer)
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    Vec<T, CPT> o;
+#pragma unroll
+    for (int j = 0; j < CPT; ++j) o.v[j] = f[j][i];
+    *reinterpret_cast<Vec<T, CPT>*>(Sn + i * ps + c0) = o;
+  }
+  if constexpr (DDF) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      Vec<T, CPT> o;
+#pragma unroll
+      for (int j = 0; j < CPT; ++j) o.v[j] = g[j][i];
+      *reinterpret_cast<Vec<T, CPT>*>(Sn + (PL::G0 + i) * ps + c0) = o;
+    }
+  }
+  if constexpr (NUMEQ) {
+#pragma unroll
+    for (int k = 0; k < NLAMBDA; ++k) {
+      Vec<T, CPT> o;
+#pragma unroll
+      for (int j = 0; j < CPT; ++j) o.v[j] = lam[j][k];
+      *reinterpret_cast<Vec<T, CPT>*>(Sn + (PL::L0 + k) * ps + c0) = o;
     }
   }
 }
@@ -397,6 +446,7 @@ __global__ void __launch_bounds__(128) macroscopic_kernel(const MacroArgs a, con
 // ------------------------------------------------------------------ dispatch table entry
 struct KernelSet {
   int Q, precision, collision, ddf, sensor;
+  int cells_per_thread;
   const char* name;
   const void* sweep;
   const void* init;
@@ -408,6 +458,7 @@ template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
 KernelSet make_kernel_set(const char* name) {
   KernelSet k;
   k.Q = Q; k.precision = (int)sizeof(T) * 8; k.collision = COLL; k.ddf = DDF; k.sensor = SENSOR;
+  k.cells_per_thread = cells_per_thread<Q, T, COLL, DDF>;
   k.name = name;
   k.sweep = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR>;
   k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;

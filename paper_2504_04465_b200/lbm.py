@@ -24,7 +24,7 @@ _ERR = {EINVAL: "LBM_EINVAL", ENOMEM: "LBM_ENOMEM", EMESH: "LBM_EMESH", ECUDA: "
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
            "lbm_get_schedule", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_sync", "lbm_get_macroscopic",
-           "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name"]
+           "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_measure_fma_peak"]
 
 
 class LbmError(RuntimeError):
@@ -84,8 +84,16 @@ def lib():
         L.lbm_last_step_ms.restype = C.c_double
         L.lbm_kernel_name.argtypes = [vp]
         L.lbm_kernel_name.restype = C.c_char_p
+        L.lbm_measure_fma_peak.argtypes = [C.c_int, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
     return _lib
+
+
+def measure_fma_peak(precision=64, seconds=1.0):
+    """lbm_measure_fma_peak: (TFLOP/s, FMA lanes x MHz per SM) of the current device's plain fp64 / fp32 pipe."""
+    tf, lm = C.c_double(0.0), C.c_double(0.0)
+    _check("lbm_measure_fma_peak", lib().lbm_measure_fma_peak(int(precision), float(seconds), C.byref(tf), C.byref(lm)))
+    return tf.value, lm.value
 
 
 def _ptr(a):
