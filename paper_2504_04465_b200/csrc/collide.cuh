@@ -70,6 +70,43 @@ __device__ __forceinline__ T poly_i(const T (&a)[NA]) {
   return s;
 }
 
+// Order of the Hermite moment in slot k (parity decides the sign under xi -> -xi).
+__host__ __device__ constexpr int slot_order(int k) { return k == A0 ? 0 : k <= AY ? 1 : k <= AYY ? 2 : k <= AYYY ? 3 : 4; }
+
+// f_I and f_opp(I) of Eq. 33/34 together: the even-order part is shared, the odd-order part changes sign
+// (H^(n)(-xi) = (-1)^n H^(n)(xi), w_opp = w), which halves the multiply-adds of the reconstruction.
+template <int Q, typename T, int I>
+__device__ __forceinline__ void poly_pair(const T (&a)[NA], T& fi, T& fo) {
+  constexpr double c0 = hermite_coef(Lat<Q>::t, I, A0);
+  T e = T(c0) * a[A0], o = T(0);
+  static_for<1, NA>([&](auto kc) {
+    constexpr int K = decltype(kc)::value;
+    constexpr double c = hermite_coef(Lat<Q>::t, I, K);
+    if constexpr (c != 0.0) {
+      if constexpr (slot_order(K) % 2 == 1) o += T(c) * a[K];
+      else e += T(c) * a[K];
+    }
+  });
+  fi = e + o;
+  fo = e - o;
+}
+
+// fn(I, fe_I) for every direction, evaluated pairwise
+template <int Q, typename T, class F>
+__device__ __forceinline__ void poly_all(const T (&a)[NA], F&& fn) {
+  fn(std::integral_constant<int, 0>{}, poly_i<Q, T, 0>(a));
+  static_for<1, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int O = Lat<Q>::t.opp[I];
+    if constexpr (O > I) {
+      T fi, fo;
+      poly_pair<Q, T, I>(a, fi, fo);
+      fn(std::integral_constant<int, I>{}, fi);
+      fn(std::integral_constant<int, O>{}, fo);
+    }
+  });
+}
+
 // rho, u (a2) and T by Eq. 51 (thermal models) or T0 = c_s^2 (athermal)
 template <int Q, typename T, bool THERMAL, bool DDF>
 __device__ __forceinline__ void moments(const ModelParams& p, const T (&f)[Q], const T (&g)[Q], T& rho, T& ux, T& uy, T& Tm) {
@@ -241,7 +278,7 @@ __device__ __forceinline__ int equilibrium(const ModelParams& p, T rho, T ux, T 
   } else {
     T a[NA];
     aeq_moments<T>(rho, ux, uy, DDF ? Tm - T(cs2_v<Q>) : T(0), a);
-    static_for<0, Q>([&](auto ic) { constexpr int I = decltype(ic)::value; feq[I] = poly_i<Q, T, I>(a); });
+    poly_all<Q, T>(a, [&](auto ic, T fe) { feq[decltype(ic)::value] = fe; });
   }
   if constexpr (DDF) {
     const T fac = T(2.0 / (p.gamma - 1.0) - 2.0) * Tm;   // Eq. 50: (2 C_v - D) T, D = 2
@@ -300,9 +337,8 @@ __device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T
     T a[NA];
     aeq_moments<T>(rho, ux, uy, DDF ? Tm - T(cs2_v<Q>) : T(0), a);
     const T fac = DDF ? T(2.0 / (p.gamma - 1.0) - 2.0) * Tm : T(0);
-    static_for<0, Q>([&](auto ic) {
+    poly_all<Q, T>(a, [&](auto ic, T fe) {
       constexpr int I = decltype(ic)::value;
-      const T fe = poly_i<Q, T, I>(a);
       f[I] = fe + keep * (f[I] - fe);
       if constexpr (DDF) { const T ge = fac * fe; g[I] = ge + keep * (g[I] - ge); }
     });
@@ -311,16 +347,31 @@ __device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T
     constexpr double c2 = cs2_v<Q>;
     T ae[NA];
     aeq_moments<T>(rho, ux, uy, T(0), ae);
-    // Pi = sum_i H_i^(2) (f_i - f_i^eq)
+    // Pi = sum_i H_i^(2) (f_i - f_i^eq).  The lattices with rational weights reproduce the second-order
+    // moments of f^eq exactly, so Pi = sum_i xi xi f_i - rho c_s^2 delta - rho u u there (one pass over f, no f^eq);
+    // D2Q37's 15-digit weights (S23) do so only to ~1e-13, so it keeps the literal form.
     T pxx = T(0), pxy = T(0), pyy = T(0);
-    static_for<0, Q>([&](auto ic) {
-      constexpr int I = decltype(ic)::value;
-      constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
-      const T dn = f[I] - poly_i<Q, T, I>(ae);
-      pxx += T(cx * cx - c2) * dn;
-      if constexpr (cx * cy != 0) pxy += T(cx * cy) * dn;
-      pyy += T(cy * cy - c2) * dn;
-    });
+    if constexpr (Q != 37) {
+      static_for<1, Q>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
+        if constexpr (cx != 0) pxx += T(cx * cx) * f[I];
+        if constexpr (cx * cy != 0) pxy += T(cx * cy) * f[I];
+        if constexpr (cy != 0) pyy += T(cy * cy) * f[I];
+      });
+      pxx = (pxx - T(c2) * rho) - ae[AXX];
+      pxy = pxy - ae[AXY];
+      pyy = (pyy - T(c2) * rho) - ae[AYY];
+    } else {
+      static_for<0, Q>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
+        const T dn = f[I] - poly_i<Q, T, I>(ae);
+        pxx += T(cx * cx - c2) * dn;
+        if constexpr (cx * cy != 0) pxy += T(cx * cy) * dn;
+        pyy += T(cy * cy - c2) * dn;
+      });
+    }
     if (p.trace_eq) {   // trace relaxes with tau = 1: only the deviatoric part survives (S7)
       const T dev = T(0.5) * (pxx - pyy);
       pxx = dev; pyy = -dev;
@@ -340,7 +391,7 @@ __device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T
     an[AYYYY] = T(4) * uy * an[AYYY] - T(6) * uy * uy * pyy;
 #pragma unroll
     for (int k = 0; k < NA; ++k) ae[k] += keep * an[k];                       // a* = a_eq + (1 - 1/tau) a_neq
-    static_for<0, Q>([&](auto ic) { constexpr int I = decltype(ic)::value; f[I] = poly_i<Q, T, I>(ae); });   // Eq. 33
+    poly_all<Q, T>(ae, [&](auto ic, T fs) { f[decltype(ic)::value] = fs; });   // Eq. 33
   }
   return it;
 }
