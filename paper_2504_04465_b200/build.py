@@ -19,7 +19,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 CU = ["lbm_api.cu", "peak.cu", "sweep_q9.cu", "sweep_q13.cu", "sweep_q21.cu", "sweep_q37.cu"]
 CPP = ["grid_builder.cpp"]
-HEADERS = [os.path.join(CSRC, h) for h in ("grid.hpp", "lattice.cuh", "collide.cuh", "sweep.cuh")] + [os.path.join(INCLUDE, "lbm.h")]
+HEADERS = sorted(os.path.join(CSRC, h) for h in os.listdir(CSRC) if h.endswith((".cuh", ".hpp", ".h"))) + [os.path.join(INCLUDE, "lbm.h")]
 
 NVCC = os.environ.get("NVCC", "nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]

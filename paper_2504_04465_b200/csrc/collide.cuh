@@ -21,6 +21,20 @@ struct ModelParams {
 
 enum { FLAG_UNSTABLE = 1, FLAG_NEWTON = 2 };
 
+// 1/x to within ~1 ulp for normal x: hardware seed (MUFU.RCP64H, ~20 bits) + two Newton steps (4 DFMA) instead
+// of the IEEE division routine (~25 instructions and a call); used where Q quotients per cell are summed (Eq. 52).
+__device__ __forceinline__ double fast_rcp(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-x, r, 1.0);
+  return fma(r, e, r);
+}
+__device__ __forceinline__ float fast_rcp(float x) { return 1.0f / x; }
+__device__ __forceinline__ void opaque(double& x) { asm volatile("" : "+d"(x)); }
+__device__ __forceinline__ void opaque(float& x) { asm volatile("" : "+f"(x)); }
+
 template <typename T> struct Num;
 template <> struct Num<double> {
   static __device__ __forceinline__ double tiny() { return 1e-300; }
@@ -288,6 +302,26 @@ __device__ __forceinline__ int equilibrium(const ModelParams& p, T rho, T ux, T 
   return it;
 }
 
+// Eq. 37-38 (typo of P:876 repaired, S2): non-equilibrium Hermite moments of orders 3-4 from Pi by the recursion,
+// then a* = a_eq + (1 - 1/tau) a_neq in place (Eq. 33).  Slots outside the lattice's basis are ignored downstream.
+template <typename T>
+__device__ __forceinline__ void rr_post_collision_moments(T ux, T uy, T pxx, T pxy, T pyy, T keep, T (&ae)[NA]) {
+  T an[NA];
+  an[A0] = T(0); an[AX] = T(0); an[AY] = T(0);
+  an[AXX] = pxx; an[AXY] = pxy; an[AYY] = pyy;
+  an[AXXX] = T(3) * ux * pxx;
+  an[AXXY] = T(2) * ux * pxy + uy * pxx;
+  an[AXYY] = T(2) * uy * pxy + ux * pyy;
+  an[AYYY] = T(3) * uy * pyy;
+  an[AXXXX] = T(4) * ux * an[AXXX] - T(6) * ux * ux * pxx;
+  an[AXXXY] = (T(3) * ux * an[AXXY] + uy * an[AXXX]) - T(3) * ux * ux * pxy - T(3) * ux * uy * pxx;
+  an[AXXYY] = T(2) * (ux * an[AXYY] + uy * an[AXXY]) - ux * ux * pyy - uy * uy * pxx - T(4) * ux * uy * pxy;
+  an[AXYYY] = (T(3) * uy * an[AXYY] + ux * an[AYYY]) - T(3) * uy * uy * pxy - T(3) * ux * uy * pyy;
+  an[AYYYY] = T(4) * uy * an[AYYY] - T(6) * uy * uy * pyy;
+#pragma unroll
+  for (int k = 0; k < NA; ++k) ae[k] += keep * an[k];
+}
+
 // Eq. 53 with reading S10: alpha = 1 below 0.01; last case alpha = 1/tau (tau_eff = 1)
 template <typename T>
 __device__ __forceinline__ T sensor_alpha(T eps, T A, T tau) {
@@ -308,10 +342,10 @@ __device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T
   rho_out = rho;
   int it = 0;
 
-  if constexpr (COLL == LBM_NUMEQ || SENSOR) {
-    // equilibrium held in registers: Newton needs it; the sensor needs all of it before relaxing
-    T feq[Q], geq[Q];
-    it = equilibrium<Q, T, COLL, DDF>(p, rho, ux, uy, Tm, lam, feq, geq);
+  if constexpr (COLL == LBM_NUMEQ) {
+    // numerical equilibrium: held in registers (Newton produces all of it; the sensor needs all of it before relaxing)
+    T feq[Q];
+    it = feq_numerical<Q, T>(p, rho, ux, uy, Tm, lam, feq);
     T tau_eff = tau;
     if constexpr (SENSOR) {
       T eps = T(0);
@@ -319,23 +353,40 @@ __device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T
       for (int i = 0; i < Q; ++i) {
         T den = Num<T>::abs_(feq[i]);
         if (den < Num<T>::tiny()) den = Num<T>::tiny();
-        eps += Num<T>::abs_(f[i] - feq[i]) / den;          // Eq. 52
+        eps += Num<T>::abs_(f[i] - feq[i]) * fast_rcp(den);          // Eq. 52
       }
       eps /= T(Q);
       tau_eff = tau * sensor_alpha<T>(eps, T(p.sensor_A), tau);
     }
     const T keep = T(1) - T(1) / tau_eff;
-    static_assert(COLL != LBM_RR || !SENSOR, "sensor is instantiated for BGK-type relaxation only");
 #pragma unroll
     for (int i = 0; i < Q; ++i) f[i] = feq[i] + keep * (f[i] - feq[i]);      // Eq. 30
     if constexpr (DDF) {
+      const T fac = T(2.0 / (p.gamma - 1.0) - 2.0) * Tm;                     // Eq. 50: (2 C_v - D) T
 #pragma unroll
-      for (int i = 0; i < Q; ++i) g[i] = geq[i] + keep * (g[i] - geq[i]);
+      for (int i = 0; i < Q; ++i) { const T ge = fac * feq[i]; g[i] = ge + keep * (g[i] - ge); }
     }
   } else if constexpr (COLL == LBM_BGK) {
-    const T keep = T(1) - T(1) / tau;
+    static_assert(COLL != LBM_RR || !SENSOR, "sensor is instantiated for BGK-type relaxation only");
+    T keep = T(1) - T(1) / tau;
     T a[NA];
     aeq_moments<T>(rho, ux, uy, DDF ? Tm - T(cs2_v<Q>) : T(0), a);
+    if constexpr (SENSOR) {
+      // Eq. 52-53 need every f_i^eq before any relaxation: one pass for eps, then f^eq is RECOMPUTED in the relaxation
+      // pass instead of being kept in Q more registers (D2Q37+g: 255 registers and spills otherwise).  The moments are
+      // hidden from common-subexpression elimination, which would undo exactly that.
+      T eps = T(0);
+      poly_all<Q, T>(a, [&](auto ic, T fe) {
+        constexpr int I = decltype(ic)::value;
+        T den = Num<T>::abs_(fe);
+        if (den < Num<T>::tiny()) den = Num<T>::tiny();
+        eps += Num<T>::abs_(f[I] - fe) * fast_rcp(den);                      // Eq. 52
+      });
+      eps /= T(Q);
+      keep = T(1) - T(1) / (tau * sensor_alpha<T>(eps, T(p.sensor_A), tau));
+#pragma unroll
+      for (int k = 0; k < NA; ++k) opaque(a[k]);
+    }
     const T fac = DDF ? T(2.0 / (p.gamma - 1.0) - 2.0) * Tm : T(0);
     poly_all<Q, T>(a, [&](auto ic, T fe) {
       constexpr int I = decltype(ic)::value;
@@ -376,21 +427,7 @@ __device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T
       const T dev = T(0.5) * (pxx - pyy);
       pxx = dev; pyy = -dev;
     }
-    // Eq. 37-38 (typo of P:876 repaired, S2)
-    T an[NA];
-    an[A0] = T(0); an[AX] = T(0); an[AY] = T(0);
-    an[AXX] = pxx; an[AXY] = pxy; an[AYY] = pyy;
-    an[AXXX] = T(3) * ux * pxx;
-    an[AXXY] = T(2) * ux * pxy + uy * pxx;
-    an[AXYY] = T(2) * uy * pxy + ux * pyy;
-    an[AYYY] = T(3) * uy * pyy;
-    an[AXXXX] = T(4) * ux * an[AXXX] - T(6) * ux * ux * pxx;
-    an[AXXXY] = (T(3) * ux * an[AXXY] + uy * an[AXXX]) - T(3) * ux * ux * pxy - T(3) * ux * uy * pxx;
-    an[AXXYY] = T(2) * (ux * an[AXYY] + uy * an[AXXY]) - ux * ux * pyy - uy * uy * pxx - T(4) * ux * uy * pxy;
-    an[AXYYY] = (T(3) * uy * an[AXYY] + ux * an[AYYY]) - T(3) * uy * uy * pxy - T(3) * ux * uy * pyy;
-    an[AYYYY] = T(4) * uy * an[AYYY] - T(6) * uy * uy * pyy;
-#pragma unroll
-    for (int k = 0; k < NA; ++k) ae[k] += keep * an[k];                       // a* = a_eq + (1 - 1/tau) a_neq
+    rr_post_collision_moments<T>(ux, uy, pxx, pxy, pyy, keep, ae);
     poly_all<Q, T>(ae, [&](auto ic, T fs) { f[decltype(ic)::value] = fs; });   // Eq. 33
   }
   return it;

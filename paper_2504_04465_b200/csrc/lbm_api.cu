@@ -101,17 +101,17 @@ const KernelSet* find_kernel_set(const lbm_config& c) {
 
 // n work items, `per_thread` of them per thread.  pdl: chain to the previous kernel of the stream with a programmatic
 // dependent-launch edge (only for kernels that call griddepcontrol.wait before touching mutable data: the sweep).
-int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s, int per_thread = 1, bool pdl = false) {
+int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s, int per_thread = 1, bool pdl = false, int smem = 0) {
   if (n <= 0) return LBM_OK;
   void* args[2] = {a0, a1};
   const int64_t threads = (n + per_thread - 1) / per_thread;
   const unsigned grid = (unsigned)((threads + BLOCK - 1) / BLOCK);
   if (!pdl) {
-    CK(cudaLaunchKernel(fn, dim3(grid), dim3(BLOCK), args, 0, s));
+    CK(cudaLaunchKernel(fn, dim3(grid), dim3(BLOCK), args, (size_t)smem, s));
     return LBM_OK;
   }
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = s;
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(BLOCK); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = s;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
