@@ -149,20 +149,62 @@ __device__ __forceinline__ void moments(const ModelParams& p, const T (&f)[Q], c
 }
 
 // ------------------------------------------------------------------ numerical equilibrium
-// f_i(lambda) = rho exp[-(1 + sum_a lambda_a M_ia)] (Eq. 39 with a = rho); G_a = sum_i f_i M_ia - m_a
+// x^N for a compile-time N >= 0 by binary exponentiation (identical sub-powers are shared by the compiler)
+template <int N, typename T>
+__device__ __forceinline__ T ipow(T x) {
+  if constexpr (N == 0) return T(1);
+  else if constexpr (N == 1) return x;
+  else if constexpr (N % 2 == 0) { const T h = ipow<N / 2, T>(x); return h * h; }
+  else return ipow<N - 1, T>(x) * x;
+}
+
+// f_i(lambda) = rho exp[-(1 + sum_a lambda_a M_ia)] (Eq. 39 with a = rho); G_a = sum_i f_i M_ia - m_a.
+// fp32: one expf per direction.  fp64: the lattice velocities are small integers, so the exponential factorises,
+//   f(x,y) = [rho e^{-1-l0}] (e^{-l3})^{x^2} (e^{-l5})^{y^2} (e^{-l4})^{xy} [e^{-l1} (e^{-l6})^{r^2}]^x [e^{-l2} (e^{-l7})^{r^2}]^y,
+// into 8 exponentials, integer powers and a few reciprocals (negative x, y, xy) per evaluation instead of Q
+// exponentials of ~20 DFMA each: the solve is fp64-ALU-bound and the exponentials were about half of its arithmetic
+// (profiles/r01_ncu_naca_f64.md).  Each f_i carries a few ulp more rounding error than exp of the summed exponent;
+// the Newton floor stays ~1e-13 rho, below the tolerance of P:934.
 template <int Q, typename T>
 __device__ __forceinline__ void numeq_eval(T rho, const T (&m)[NLAMBDA], const T (&lam)[NLAMBDA], T (&f)[Q], T (&G)[NLAMBDA]) {
 #pragma unroll
   for (int a = 0; a < NLAMBDA; ++a) G[a] = T(0);
+  [[maybe_unused]] T C, ea, eb, ec, eci, ep, eq, es, et;
+  if constexpr (sizeof(T) == 8) {
+    C = rho * Num<T>::exp_(-(T(1) + lam[0]));
+    ep = Num<T>::exp_(-lam[1]); eq = Num<T>::exp_(-lam[2]);
+    ea = Num<T>::exp_(-lam[3]); ec = Num<T>::exp_(-lam[4]); eb = Num<T>::exp_(-lam[5]);
+    es = Num<T>::exp_(-lam[6]); et = Num<T>::exp_(-lam[7]);
+    eci = fast_rcp(ec);
+  }
   static_for<0, Q>([&](auto ic) {
     constexpr int I = decltype(ic)::value;
-    T e = T(1);
-    static_for<0, NLAMBDA>([&](auto ac) {
-      constexpr int A = decltype(ac)::value;
-      constexpr int M = monomial(Lat<Q>::t, I, A);
-      if constexpr (M != 0) e += lam[A] * T(M);
-    });
-    const T fi = rho * Num<T>::exp_(-e);
+    T fi;
+    if constexpr (sizeof(T) == 8) {
+      constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I], r2 = x * x + y * y;
+      constexpr int ax = x < 0 ? -x : x, ay = y < 0 ? -y : y, axy = x * y < 0 ? -x * y : x * y;
+      fi = C;
+      if constexpr (x != 0) fi *= ipow<x * x, T>(ea);
+      if constexpr (y != 0) fi *= ipow<y * y, T>(eb);
+      if constexpr (x * y > 0) fi *= ipow<axy, T>(ec);
+      if constexpr (x * y < 0) fi *= ipow<axy, T>(eci);
+      if constexpr (x != 0) {
+        const T X = ipow<ax, T>(ep * ipow<r2, T>(es));
+        fi *= x > 0 ? X : fast_rcp(X);
+      }
+      if constexpr (y != 0) {
+        const T Y = ipow<ay, T>(eq * ipow<r2, T>(et));
+        fi *= y > 0 ? Y : fast_rcp(Y);
+      }
+    } else {
+      T e = T(1);
+      static_for<0, NLAMBDA>([&](auto ac) {
+        constexpr int A = decltype(ac)::value;
+        constexpr int M = monomial(Lat<Q>::t, I, A);
+        if constexpr (M != 0) e += lam[A] * T(M);
+      });
+      fi = rho * Num<T>::exp_(-e);
+    }
     f[I] = fi;
     static_for<0, NLAMBDA>([&](auto ac) {
       constexpr int A = decltype(ac)::value;
@@ -243,41 +285,38 @@ __device__ __forceinline__ int feq_numerical(const ModelParams& p, T rho, T ux, 
   // right-hand sides of Eq. 42-49 with 2E = u^2 + 2T
   const T m[NLAMBDA] = {rho, rho * ux, rho * uy, rho * (ux * ux + Tm), rho * ux * uy, rho * (uy * uy + Tm),
                         rho * ux * (u2 + T(4) * Tm), rho * uy * (u2 + T(4) * Tm)};
+  // One loop with a single evaluation site and a single direction site (the three textual call sites of the rule --
+  // initial residual, line-search trial, polish -- are phases of it): fully inlined, each site is ~1-2 k instructions,
+  // and three copies of them overflowed the instruction cache (profiles/r01_ncu_naca_f64.md: stall_no_instruction).
   T G[NLAMBDA], d[NLAMBDA], lt[NLAMBDA];
   const T tol = T(p.newton_tol) * rho;
-  int it = 0;
+  enum { INIT, SEARCH, POLISH };
+  int it = 0, phase = INIT;
   bool converged = false, bad = false;
-  numeq_eval<Q, T>(rho, m, lam, f, G);
+  T t = T(0), n0 = T(0);
+#pragma unroll
+  for (int a = 0; a < NLAMBDA; ++a) d[a] = T(0);
+#pragma unroll 1
   for (;;) {
-    T r1 = T(0);
 #pragma unroll
-    for (int a = 0; a < NLAMBDA; ++a) r1 += Num<T>::abs_(G[a]);
-    if (r1 <= tol) { converged = true; break; }
-    if (it >= p.newton_max_iter) break;
-    if (!newton_direction<Q, T>(f, G, d)) { bad = true; break; }
-    const T n0 = norm2sq(G);
-    T t = T(1);
-    for (;;) {
-#pragma unroll
-      for (int a = 0; a < NLAMBDA; ++a) lt[a] = lam[a] + t * d[a];
-      numeq_eval<Q, T>(rho, m, lt, f, G);
+    for (int a = 0; a < NLAMBDA; ++a) lt[a] = lam[a] + t * d[a];
+    numeq_eval<Q, T>(rho, m, lt, f, G);
+    if (phase == SEARCH) {
       const T n1 = norm2sq(G);
-      if (n1 < n0 || t <= T(1.0 / 1024.0)) break;   // a NaN norm fails the first test and keeps halving
-      t *= T(0.5);
+      if (!(n1 < n0) && t > T(1.0 / 1024.0)) { t *= T(0.5); continue; }   // a NaN norm keeps halving
     }
 #pragma unroll
     for (int a = 0; a < NLAMBDA; ++a) lam[a] = lt[a];
-    ++it;
-  }
-  if (!bad) {   // polish
-    if (newton_direction<Q, T>(f, G, d)) {
+    if (phase != INIT) ++it;
+    if (phase == POLISH) break;
+    T r1 = T(0);
 #pragma unroll
-      for (int a = 0; a < NLAMBDA; ++a) lam[a] += d[a];
-      numeq_eval<Q, T>(rho, m, lam, f, G);
-      ++it;
-    } else {
-      bad = true;
-    }
+    for (int a = 0; a < NLAMBDA; ++a) r1 += Num<T>::abs_(G[a]);
+    converged = r1 <= tol;
+    phase = (converged || it >= p.newton_max_iter) ? POLISH : SEARCH;    // then one unconditional full Newton step
+    if (!newton_direction<Q, T>(f, G, d)) { bad = true; break; }
+    n0 = norm2sq(G);
+    t = T(1);
   }
   return (converged && !bad) ? it : -it - 1;
 }
@@ -333,12 +372,20 @@ __device__ __forceinline__ T sensor_alpha(T eps, T A, T tau) {
 
 // Steps 2-5 of the cell update, in place: f, g pre-collision in, post-collision out.
 // Returns Newton iterations (0 for polynomial models, negative on failure); rho_out = pre-collision density.
+// `imp` (numerical equilibria only): an equilibrium Dirichlet cell passes its imposed state here and receives
+// f = f^eq, g = g^eq of it, so that the kernel holds ONE inlined copy of the Newton solver (instruction-cache footprint).
+template <typename T> struct Imposed { bool on; T rho, ux, uy, Tm; };
+
 template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
-__device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T (&g)[Q], T (&lam)[NLAMBDA], T& rho_out) {
+__device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T (&g)[Q], T (&lam)[NLAMBDA], T& rho_out,
+                                       const Imposed<T> imp = Imposed<T>{false, T(0), T(0), T(0), T(0)}) {
   constexpr bool THERMAL = (COLL == LBM_NUMEQ) || DDF;
   static_assert(!(COLL == LBM_RR && DDF), "RR is defined for the athermal models only");
   T rho, ux, uy, Tm;
   moments<Q, T, THERMAL, DDF>(p, f, g, rho, ux, uy, Tm);
+  if constexpr (COLL == LBM_NUMEQ) {
+    if (imp.on) { rho = imp.rho; ux = imp.ux; uy = imp.uy; Tm = imp.Tm; }
+  }
   rho_out = rho;
   int it = 0;
 
@@ -360,11 +407,11 @@ __device__ __forceinline__ int collide(const ModelParams& p, T tau, T (&f)[Q], T
     }
     const T keep = T(1) - T(1) / tau_eff;
 #pragma unroll
-    for (int i = 0; i < Q; ++i) f[i] = feq[i] + keep * (f[i] - feq[i]);      // Eq. 30
+    for (int i = 0; i < Q; ++i) f[i] = imp.on ? feq[i] : feq[i] + keep * (f[i] - feq[i]);      // Eq. 30
     if constexpr (DDF) {
       const T fac = T(2.0 / (p.gamma - 1.0) - 2.0) * Tm;                     // Eq. 50: (2 C_v - D) T
 #pragma unroll
-      for (int i = 0; i < Q; ++i) { const T ge = fac * feq[i]; g[i] = ge + keep * (g[i] - ge); }
+      for (int i = 0; i < Q; ++i) { const T ge = fac * feq[i]; g[i] = imp.on ? ge : ge + keep * (g[i] - ge); }
     }
   } else if constexpr (COLL == LBM_BGK) {
     static_assert(COLL != LBM_RR || !SENSOR, "sensor is instantiated for BGK-type relaxation only");

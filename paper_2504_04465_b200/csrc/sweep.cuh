@@ -121,6 +121,7 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
 #pragma unroll
   for (int j = 0; j < CPT; ++j) {
     const int c = c0 + j;
+    Imposed<T> imp{false, T(0), T(0), T(0), T(0)};
     if (type[j] == LBM_DIRICHLET) {
       // equilibrium Dirichlet cell: imposed (rho,u,T); rho optionally from the nearest interior cell
       const int sd = side[j];
@@ -133,18 +134,18 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
       }
       const T Tb = (NUMEQ || DDF) ? T(p.bc_T[sd]) : T(cs2_v<Q>);
       if constexpr (NUMEQ) {
+        // falls through to the one inlined Newton solver below (warm start: the cell's own stored multipliers)
+        imp = Imposed<T>{true, rho, T(p.bc_ux[sd]), T(p.bc_uy[sd]), Tb};
+      } else {
+        T geq[Q];
+        equilibrium<Q, T, COLL, DDF>(p, rho, T(p.bc_ux[sd]), T(p.bc_uy[sd]), Tb, lam[j], f[j], geq);
+        if constexpr (DDF) {
 #pragma unroll
-        for (int k = 0; k < NLAMBDA; ++k) lam[j][k] = So[(PL::L0 + k) * ps + c];
+          for (int i = 0; i < Q; ++i) g[j][i] = geq[i];
+        }
+        if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+        continue;
       }
-      T geq[Q];
-      const int it = equilibrium<Q, T, COLL, DDF>(p, rho, T(p.bc_ux[sd]), T(p.bc_uy[sd]), Tb, lam[j], f[j], geq);
-      if constexpr (DDF) {
-#pragma unroll
-        for (int i = 0; i < Q; ++i) g[j][i] = geq[i];
-      }
-      if (it < 0) atomicOr(a.status, FLAG_NEWTON);
-      if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
-      continue;
     }
 
     bool special = false;     // any velocity-bounce-back or unknown link
@@ -152,7 +153,7 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
       constexpr int I = decltype(ic)::value;
       special |= (nb[j][I] <= LBM_LINK_VBB0) || (nb[j][I] == LBM_LINK_NONE);
     });
-    if (special) {
+    if (special && !imp.on) {
       if (type[j] == LBM_COARSE_GHOST) {
         // coalescence (Eq. 4): unknown directions only, mean over the children that exist
         const int* ch = a.g_child + 4ll * a.aux[c];
@@ -232,7 +233,7 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
 
     // ---- steps 2-5: moments, equilibrium, sensor, relaxation
     T rho;
-    const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f[j], g[j], lam[j], rho);
+    const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f[j], g[j], lam[j], rho, imp);
     if (it < 0) atomicOr(a.status, FLAG_NEWTON);
     if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
 
