@@ -134,6 +134,11 @@ int lbm_init_fields(lbm_grid* g, const double* rho, const double* ux, const doub
 /* Enqueues n_coarse_steps coarse steps (each 2^depth fine steps of the schedule above) on the bound
  * stream and returns without synchronising. */
 int lbm_step(lbm_grid* g, int n_coarse_steps);
+/* Enqueues n FINE steps of the same schedule (fine step k updates level 0, then every level l with k = 0 mod 2^l,
+ * ascending; listing P:202-215 in pull form) as plain kernel launches, continuing from wherever the previous call
+ * stopped inside the coarse step.  For tests and for timing sub-steps; lbm_step returns LBM_ESTATE unless the
+ * fine-step count since the last coarse-step boundary is a multiple of 2^depth.  lbm_init_fields resets the count. */
+int lbm_step_fine(lbm_grid* g, int n_fine_steps);
 /* Waits for the stream and returns the sticky device status: LBM_OK, LBM_EUNSTABLE or LBM_ENEWTON. */
 int lbm_sync(lbm_grid* g);
 

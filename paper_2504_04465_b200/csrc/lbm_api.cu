@@ -70,6 +70,7 @@ struct lbm_grid {
   cudaGraphExec_t g1[2] = {nullptr, nullptr};     // one coarse step, starting parity of the coarsest level
   cudaGraphExec_t gk[2] = {nullptr, nullptr};     // K coarse steps (K even), for launch-bound small grids
   int K = 0;
+  int64_t kfine = 0;                              // fine steps taken inside the current coarse step (lbm_step_fine)
   cudaEvent_t ev0 = nullptr, ev1 = nullptr;
   bool timed = false;
 };
@@ -431,12 +432,36 @@ int lbm_init_fields(lbm_grid* g, const double* rho, const double* ux, const doub
   }
   g->inited = true;
   g->timed = false;
+  g->kfine = 0;
   return status_code(g);
+}
+
+int lbm_step_fine(lbm_grid* g, int n) {
+  if (!g || n < 0) return LBM_EINVAL;
+  if (!g->bound || !g->inited) return LBM_ESTATE;
+  const int d = g->depth;
+  std::vector<int> cur((size_t)d + 1);
+  for (int l = 0; l <= d; ++l) cur[l] = g->dl[l].cur;
+  CK(cudaEventRecord(g->ev0, g->stream));
+  for (int s = 0; s < n; ++s) {
+    const int64_t k = g->kfine + 1;               // schedule of DESIGN.md Sec. 6 rule 9 at fine step k
+    for (int l = 0; l <= d; ++l) {
+      if (l > 0 && (k % ((int64_t)1 << l)) != 0) break;
+      int rc = enqueue_level(g, l, cur.data());
+      if (rc) return rc;
+    }
+    g->kfine = k % ((int64_t)1 << d);
+  }
+  CK(cudaEventRecord(g->ev1, g->stream));
+  for (int l = 0; l <= d; ++l) g->dl[l].cur = cur[l];
+  g->timed = true;
+  return LBM_OK;
 }
 
 int lbm_step(lbm_grid* g, int n) {
   if (!g || n < 0) return LBM_EINVAL;
   if (!g->bound || !g->inited) return LBM_ESTATE;
+  if (g->kfine != 0) return LBM_ESTATE;           // graphs start at a coarse-step boundary
   int& p = g->dl[g->depth].cur;
   CK(cudaEventRecord(g->ev0, g->stream));
   while (n > 0) {
