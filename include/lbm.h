@@ -88,6 +88,7 @@ typedef struct {
   int64_t launches_per_coarse_step;       /* kernels enqueued per coarse step */
   size_t  arena_bytes;                    /* device memory the caller must provide to lbm_grid_bind */
   double  tau[LBM_MAX_LEVELS];
+  int64_t n_bricks[LBM_MAX_LEVELS];       /* regular 8x8 bricks (64 cells each) addressed by tile arithmetic on the device */
 } lbm_grid_info;
 
 typedef struct lbm_grid lbm_grid;   /* opaque */
@@ -119,6 +120,14 @@ int lbm_get_cells(const lbm_grid* g, int level, int32_t* ix, int32_t* iy, int32_
 int lbm_get_nbr(const lbm_grid* g, int level, int32_t* nbr);
 int lbm_get_ghosts(const lbm_grid* g, int level, int32_t* coarse, int32_t* child, uint64_t* mask);
 int lbm_get_schedule(const lbm_grid* g, int32_t* k_of, int32_t* level_of, int cap);
+/* Compressed addressing of the device path: a "brick" is an aligned 8x8 tile of level-`level`
+ * cells that are all stored FLUID cells (hence 64 consecutive storage indices) and whose
+ * every neighbour-list entry equals  tiles9[9*b + k] + z  with (k, z) = (table[(i-1)*64 + m] >> 6, & 63) for the
+ * cell at Z-position m and direction i: k = 3*ky + kx numbers the 3x3 tiles around the brick (k = 4: itself),
+ * tiles9 holds the storage index of their first cell, z is the Z-position of the pull source in its tile.  The
+ * builder verifies every brick against the list entry by entry; cells outside bricks use the list.
+ * tiles9: HOST out, 9*n_bricks[level] int32; table: HOST out, (Q-1)*64 uint16; either may be NULL. */
+int lbm_get_bricks(const lbm_grid* g, int level, int32_t* tiles9, uint16_t* table);
 
 /* Attaches caller-owned DEVICE memory (>= arena_bytes, 256-byte aligned) and a CUDA stream
  * (cudaStream_t passed as void*; NULL = legacy default stream), uploads the mesh tables and captures

@@ -28,6 +28,12 @@ struct HostLevel {
   std::vector<int32_t> g_coarse, g_child;   // g_child: 4 per ghost
   std::vector<uint64_t> g_mask;
   double tau = 0.0;
+  // regular bricks (compressed addressing of the CUDA path): aligned 8x8 tiles of FLUID cells whose
+  // every link is reproduced by tile arithmetic.  brick_nb[9*b + k]: storage index of the first cell of the tile at
+  // offset (k%3-1, k/3-1) (k = 4: the brick itself).  irr: the cells outside bricks, ascending.
+  int64_t nbrick = 0;
+  std::vector<int32_t> brick_nb;
+  std::vector<int32_t> irr;
 };
 
 struct HostGrid {
@@ -35,6 +41,9 @@ struct HostGrid {
   Lattice lat;
   int depth = 0;
   std::vector<HostLevel> lv;
+  // brick_tab[(i-1)*64 + m] = (k << 6) | off: the pull source of direction i of the cell at Z-position m of a brick
+  // is cell `off` (Z-position) of the tile k of brick_nb.
+  std::vector<uint16_t> brick_tab;
 };
 
 // Returns LBM_OK, LBM_EINVAL, LBM_EMESH or LBM_ENOMEM.

@@ -420,6 +420,63 @@ int build_grid(const lbm_config& cfg, const int64_t* split_off, const int32_t* s
     }
     L.ng = (int64_t)L.g_coarse.size();
   }
+  // ---- (9) regular bricks: an aligned 8x8 tile whose 64 cells are stored (hence consecutive along the Z-curve), all
+  // FLUID, and whose every list entry equals base[tile of the source] + Z-position of the
+  // source inside that tile.  Each candidate is VERIFIED against the list built above, entry by entry, so the
+  // compressed addressing can never disagree with the neighbour list it replaces on the device.
+  G.brick_tab.assign((size_t)(Q - 1) * 64, 0);
+  for (int i = 1; i < Q; ++i)
+    for (int m = 0; m < 64; ++m) {
+      const int x = (int)gather_bits((uint64_t)m), y = (int)gather_bits((uint64_t)m >> 1);
+      const int sx = x - lat.cx[i], sy = y - lat.cy[i];
+      const int kx = sx < 0 ? 0 : (sx > 7 ? 2 : 1), ky = sy < 0 ? 0 : (sy > 7 ? 2 : 1);
+      G.brick_tab[(size_t)(i - 1) * 64 + m] = (uint16_t)(((kx + 3 * ky) << 6) | (int)zkey(sx & 7, sy & 7));
+    }
+  for (int l = 0; l <= d; ++l) {
+    HostLevel& L = G.lv[l];
+    const BuildLevel& b = B[l];
+    const int64_t n = L.n;
+    const size_t ntile = b.cells.bm.word.size();
+    const int tnx = b.nx / 8, tny = b.ny / 8;            // whole tiles inside the box
+    std::vector<int32_t> cand(ntile * 9, -1);
+    std::vector<uint8_t> isbrick(ntile, 0);
+    parallel_for((int64_t)ntile, [&](int64_t lo, int64_t hi) {
+      for (int64_t t = lo; t < hi; ++t) {
+        if (b.cells.bm.word[t] != ~0ull) continue;
+        const int32_t base = b.cells.base[t];
+        bool ok = true;
+        for (int m = 0; m < 64 && ok; ++m) ok = L.type[(size_t)base + m] == LBM_FLUID;
+        if (!ok) continue;
+        const int tx = (int)gather_bits((uint64_t)t), ty = (int)gather_bits((uint64_t)t >> 1);
+        int32_t* nb = &cand[(size_t)t * 9];
+        for (int k = 0; k < 9; ++k) {
+          int ux = tx + k % 3 - 1, uy = ty + k / 3 - 1;
+          if (ux < 0 || ux >= tnx) { if (!perx || b.nx % 8 != 0) continue; ux = (ux + tnx) % tnx; }
+          if (uy < 0 || uy >= tny) { if (!pery || b.ny % 8 != 0) continue; uy = (uy + tny) % tny; }
+          const uint64_t u = zkey(ux, uy);
+          if (u < ntile && b.cells.bm.word[u] == ~0ull) nb[k] = b.cells.base[u];
+        }
+        for (int i = 1; i < Q && ok; ++i)
+          for (int m = 0; m < 64; ++m) {
+            const uint16_t e = G.brick_tab[(size_t)(i - 1) * 64 + m];
+            const int32_t tb = nb[e >> 6];
+            if (tb < 0 || L.nbr[(size_t)(i - 1) * n + base + m] != tb + (e & 63)) { ok = false; break; }
+          }
+        isbrick[t] = ok ? 1 : 0;
+      }
+    });
+    std::vector<uint8_t> covered((size_t)n, 0);
+    for (size_t t = 0; t < ntile; ++t) {
+      if (!isbrick[t]) continue;
+      L.brick_nb.insert(L.brick_nb.end(), &cand[t * 9], &cand[t * 9] + 9);
+      std::fill(covered.begin() + b.cells.base[t], covered.begin() + b.cells.base[t] + 64, (uint8_t)1);
+    }
+    L.nbrick = (int64_t)(L.brick_nb.size() / 9);
+    L.irr.reserve((size_t)(n - 64 * L.nbrick));
+    for (int64_t c = 0; c < n; ++c)
+      if (!covered[(size_t)c]) L.irr.push_back((int32_t)c);
+  }
+
   // Eq. 3 (reading S3): tau_l - 1/2 = (tau_0 - 1/2) / 2^l
   for (int l = 0; l <= d; ++l) G.lv[l].tau = 0.5 + (cfg.tau0 - 0.5) / (double)((int64_t)1 << l);
   return LBM_OK;

@@ -24,6 +24,10 @@ constexpr size_t ALIGN = 256;
 struct DevLevel {
   int64_t n = 0, ps = 0, ng = 0;
   size_t off_type = 0, off_aux = 0, off_nbr = 0, off_gcoarse = 0, off_gchild = 0, off_S[2] = {0, 0};
+  size_t off_bricks = 0, off_irr = 0;
+  int64_t nbrick = 0, n_irr = 0;
+  int* brick_nb = nullptr;
+  int* irr = nullptr;
   unsigned char* type = nullptr;
   int* aux = nullptr;
   int* nbr = nullptr;
@@ -62,6 +66,9 @@ struct lbm_grid {
   int64_t n_total = 0, launches_per_coarse = 0, updates_per_coarse = 0;
   size_t arena_bytes = 0, off_status = 0, off_scratch = 0, scratch_doubles = 0;
   bool bound = false, inited = false, own_stream = false;
+  bool bricks = false;                            // compressed addressing of regular bricks (LBM_NO_BRICKS=1 disables)
+  size_t off_tab = 0;
+  unsigned short* d_tab = nullptr;
   bool pdl = true;                                // programmatic dependent launch between level sweeps (LBM_NO_PDL=1 disables)
   char* arena = nullptr;
   cudaStream_t stream = nullptr;
@@ -102,11 +109,17 @@ const KernelSet* find_kernel_set(const lbm_config& c) {
 
 // n work items, `per_thread` of them per thread.  pdl: chain to the previous kernel of the stream with a programmatic
 // dependent-launch edge (only for kernels that call griddepcontrol.wait before touching mutable data: the sweep).
+int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem = 0);
+
 int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s, int per_thread = 1, bool pdl = false, int smem = 0) {
   if (n <= 0) return LBM_OK;
-  void* args[2] = {a0, a1};
   const int64_t threads = (n + per_thread - 1) / per_thread;
-  const unsigned grid = (unsigned)((threads + BLOCK - 1) / BLOCK);
+  return launch_grid(fn, (unsigned)((threads + BLOCK - 1) / BLOCK), a0, a1, s, pdl, smem);
+}
+
+int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem) {
+  if (grid == 0) return LBM_OK;
+  void* args[2] = {a0, a1};
   if (!pdl) {
     CK(cudaLaunchKernel(fn, dim3(grid), dim3(BLOCK), args, (size_t)smem, s));
     return LBM_OK;
@@ -132,7 +145,15 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   a.fps = l > 0 ? g->dl[l - 1].ps : 0;
   a.tau = g->hg.lv[l].tau;
   a.status = g->d_status;
-  int rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream, g->ks->cells_per_thread, g->pdl);
+  a.brick_nb = L.brick_nb; a.brick_tab = g->d_tab; a.irr = L.irr;
+  a.nbrick = (int)L.nbrick; a.n_irr = (int)L.n_irr;
+  const int64_t cells_per_cta = (int64_t)BLOCK * g->ks->brick_cells_per_thread;
+  a.brick_ctas = (int)((L.nbrick * 64 + cells_per_cta - 1) / cells_per_cta);
+  int rc;
+  if (g->bricks && L.nbrick > 0)
+    rc = launch_grid(g->ks->sweep_bricks, (unsigned)(a.brick_ctas + (L.n_irr + BLOCK - 1) / BLOCK), &a, &g->mp, g->stream, g->pdl);
+  else
+    rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream, g->ks->cells_per_thread, g->pdl);
   cur[l] ^= 1;
   return rc;
 }
@@ -234,12 +255,16 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
       L.off_nbr = off; off += round_up((size_t)L.ps * 4 * (size_t)(g->Q - 1), ALIGN);
       L.off_gcoarse = off; off += round_up((size_t)std::max<int64_t>(H.ng, 1) * 4, ALIGN);
       L.off_gchild = off; off += round_up((size_t)std::max<int64_t>(H.ng, 1) * 16, ALIGN);
+      L.nbrick = H.nbrick; L.n_irr = (int64_t)H.irr.size();
+      L.off_bricks = off; off += round_up((size_t)std::max<int64_t>(H.nbrick, 1) * 36, ALIGN);
+      L.off_irr = off; off += round_up((size_t)std::max<int64_t>(L.n_irr, 1) * 4, ALIGN);
       for (int b = 0; b < 2; ++b) { L.off_S[b] = off; off += round_up((size_t)L.ps * (size_t)g->npop * (size_t)g->esize, ALIGN); }
       g->n_total += H.n;
       nmax = std::max(nmax, H.n);
       g->updates_per_coarse += H.n << (g->depth - l);
       g->launches_per_coarse += (H.n > 0 ? 1 : 0) * ((int64_t)1 << (g->depth - l));
     }
+    g->off_tab = off; off += round_up(g->hg.brick_tab.size() * 2, ALIGN);
     g->scratch_doubles = (size_t)std::max<int64_t>(4 * g->n_total, nmax * std::max(g->Q, LBM_NLAMBDA)) + 8;
     g->off_scratch = off; off += round_up(g->scratch_doubles * 8, ALIGN);
     g->arena_bytes = off;
@@ -274,6 +299,7 @@ int lbm_grid_query(const lbm_grid* g, lbm_grid_info* o) {
     const HostLevel& H = g->hg.lv[l];
     o->n_cells[l] = H.n; o->n_inbox[l] = H.n_inbox; o->n_coarse_ghosts[l] = H.ng; o->n_fine_ghosts[l] = H.n_fine_ghost;
     o->tau[l] = H.tau;
+    o->n_bricks[l] = H.nbrick;
   }
   o->n_total = g->n_total;
   o->updates_per_coarse_step = g->updates_per_coarse;
@@ -309,6 +335,14 @@ int lbm_get_ghosts(const lbm_grid* g, int l, int32_t* coarse, int32_t* child, ui
   if (coarse) memcpy(coarse, H.g_coarse.data(), sizeof(int32_t) * (size_t)H.ng);
   if (child) memcpy(child, H.g_child.data(), sizeof(int32_t) * (size_t)(4 * H.ng));
   if (mask) memcpy(mask, H.g_mask.data(), sizeof(uint64_t) * (size_t)H.ng);
+  return LBM_OK;
+}
+
+int lbm_get_bricks(const lbm_grid* g, int l, int32_t* tiles9, uint16_t* table) {
+  if (!g || l < 0 || l > g->depth) return LBM_EINVAL;
+  const HostLevel& H = g->hg.lv[l];
+  if (tiles9 && H.nbrick > 0) memcpy(tiles9, H.brick_nb.data(), sizeof(int32_t) * (size_t)(9 * H.nbrick));
+  if (table) memcpy(table, g->hg.brick_tab.data(), sizeof(uint16_t) * g->hg.brick_tab.size());
   return LBM_OK;
 }
 
@@ -363,6 +397,10 @@ int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream
     CK(cudaMemcpyAsync(L.aux, H.aux.data(), (size_t)H.n * 4, cudaMemcpyHostToDevice, g->stream));
     CK(cudaMemcpy2DAsync(L.nbr, (size_t)L.ps * 4, H.nbr.data(), (size_t)H.n * 4, (size_t)H.n * 4, (size_t)(Q - 1),
                          cudaMemcpyHostToDevice, g->stream));
+    L.brick_nb = (int*)(g->arena + L.off_bricks);
+    L.irr = (int*)(g->arena + L.off_irr);
+    if (H.nbrick > 0) CK(cudaMemcpyAsync(L.brick_nb, H.brick_nb.data(), (size_t)H.nbrick * 36, cudaMemcpyHostToDevice, g->stream));
+    if (!H.irr.empty()) CK(cudaMemcpyAsync(L.irr, H.irr.data(), H.irr.size() * 4, cudaMemcpyHostToDevice, g->stream));
     if (H.ng > 0) {
       CK(cudaMemcpyAsync(L.g_coarse, H.g_coarse.data(), (size_t)H.ng * 4, cudaMemcpyHostToDevice, g->stream));
       CK(cudaMemcpyAsync(L.g_child, H.g_child.data(), (size_t)H.ng * 16, cudaMemcpyHostToDevice, g->stream));
@@ -370,11 +408,15 @@ int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream
     // padding of the population planes is never read by a valid link; zero it once so that exports are clean
     for (int b = 0; b < 2; ++b) CK(cudaMemsetAsync(L.S[b], 0, (size_t)L.ps * g->npop * g->esize, g->stream));
   }
+  g->d_tab = (unsigned short*)(g->arena + g->off_tab);
+  CK(cudaMemcpyAsync(g->d_tab, g->hg.brick_tab.data(), g->hg.brick_tab.size() * 2, cudaMemcpyHostToDevice, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   CK(cudaEventCreate(&g->ev0));
   CK(cudaEventCreate(&g->ev1));
   g->bound = true;
   if (const char* e = getenv("LBM_NO_PDL")) g->pdl = !(e[0] == '1');
+  g->bricks = g->ks->sweep_bricks != nullptr;
+  if (const char* e = getenv("LBM_NO_BRICKS")) g->bricks = g->bricks && !(e[0] == '1');
   // graphs: one coarse step from either parity of the coarsest level, and K steps for launch-bound grids
   for (int p = 0; p < 2; ++p) {
     int rc = capture(g, p, 1, &g->g1[p]);

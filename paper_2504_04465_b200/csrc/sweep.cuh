@@ -35,6 +35,12 @@ struct LevelArgs {
   long long fps;            // its plane stride
   double tau;
   int* status;              // sticky FLAG_* word
+  // compressed addressing (BRICKS kernels): the first brick_ctas CTAs update regular bricks through tile arithmetic,
+  // the others the n_irr remaining cells irr[] through the list
+  const int* brick_nb;      // [nbrick][9] first storage index of the 3x3 tiles around (and of, k = 4) the brick
+  const unsigned short* brick_tab;   // [(Q-1)][64] (k << 6) | Z-position of the pull source
+  const int* irr;
+  int nbrick, n_irr, brick_ctas;
 };
 
 template <int Q, bool DDF, int COLL>
@@ -62,14 +68,87 @@ template <typename T, int N> struct alignas(sizeof(T) * N) Vec { T v[N]; };
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
+// Models whose regular interior is updated through bricks (weakly compressible, one population set).
+template <int Q, typename T, int COLL, bool DDF>
+constexpr bool has_bricks = !DDF && COLL != LBM_NUMEQ && Q <= 21;
+
+// Regular-brick path: 64 consecutive cells = one aligned 8x8 tile of fluid cells whose pull sources are
+// base[tile k] + Z-position, (k, Z-position) from a 64-entry table per direction (computed
+// addressing in regular interiors).  Replaces (Q-1) x 4 B of list and the type byte per cell by 36 B per 64 cells.
+template <int Q, typename T, int COLL>
+__device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelParams& p) {
+  constexpr int CPT = sizeof(T) == 4 ? 2 : 1;
+  constexpr int BPC = 128 * CPT / 64;                       // bricks per CTA
+  const int lt = threadIdx.x * CPT;
+  const int brick = blockIdx.x * BPC + lt / 64;
+  if (brick >= a.nbrick) return;
+  const int m0 = lt % 64;
+  const int* __restrict__ nbk = a.brick_nb + 9ll * brick;
+  const int base = __ldg(nbk + 4);
+  const long long ps = a.ps;
+  int src[CPT][Q];
+#pragma unroll
+  for (int j = 0; j < CPT; ++j) {
+    src[j][0] = base + m0 + j;
+    static_for<1, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      const int e = __ldg(a.brick_tab + (I - 1) * 64 + m0 + j);
+      src[j][I] = __ldg(nbk + (e >> 6)) + (e & 63);
+    });
+  }
+  pdl_wait();
+  const T* __restrict__ So = (const T*)a.So;
+  T* __restrict__ Sn = (T*)a.Sn;
+  T f[CPT][Q], g[1][Q], lam[NLAMBDA];
+#pragma unroll
+  for (int j = 0; j < CPT; ++j)
+    static_for<0, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      f[j][I] = So[I * ps + src[j][I]];
+    });
+#pragma unroll
+  for (int j = 0; j < CPT; ++j) {
+    T rho;
+    collide<Q, T, COLL, false, false>(p, T(a.tau), f[j], g[0], lam, rho);
+    if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+  }
+  // a brick starts at any storage index: CPT-wide stores when its first cell is CPT-aligned (uniform per brick)
+  if (CPT == 1 || base % CPT == 0) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      Vec<T, CPT> o;
+#pragma unroll
+      for (int j = 0; j < CPT; ++j) o.v[j] = f[j][i];
+      *reinterpret_cast<Vec<T, CPT>*>(Sn + i * ps + base + m0) = o;
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < Q; ++i)
+#pragma unroll
+      for (int j = 0; j < CPT; ++j) Sn[i * ps + base + m0 + j] = f[j][i];
+  }
+}
+
+template <int Q, typename T, int COLL, bool DDF, bool SENSOR, bool BRICKS>
 __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep_kernel(const LevelArgs a, const ModelParams p) {
   using PL = PopLayout<Q, DDF, COLL>;
   constexpr bool NUMEQ = COLL == LBM_NUMEQ;
-  constexpr int CPT = cells_per_thread<Q, T, COLL, DDF>;
+  constexpr int CPT = BRICKS ? 1 : cells_per_thread<Q, T, COLL, DDF>;
   pdl_launch_dependents();
-  const int c0 = (blockIdx.x * blockDim.x + threadIdx.x) * CPT;
-  if (c0 >= a.n) return;
+  int c0;
+  if constexpr (BRICKS) {
+    static_assert(has_bricks<Q, T, COLL, DDF> && !SENSOR, "no brick path for this model");
+    if ((int)blockIdx.x < a.brick_ctas) {
+      brick_update<Q, T, COLL>(a, p);
+      return;
+    }
+    const int t = ((int)blockIdx.x - a.brick_ctas) * blockDim.x + threadIdx.x;
+    if (t >= a.n_irr) return;
+    c0 = a.irr[t];
+  } else {
+    c0 = (blockIdx.x * blockDim.x + threadIdx.x) * CPT;
+    if (c0 >= a.n) return;
+  }
   const T* __restrict__ So = (const T*)a.So;
   T* __restrict__ Sn = (T*)a.Sn;
   const long long ps = a.ps;
@@ -450,6 +529,8 @@ struct KernelSet {
   int cells_per_thread;
   const char* name;
   const void* sweep;
+  const void* sweep_bricks;   // same update with compressed addressing of regular bricks, or null
+  int brick_cells_per_thread;
   const void* init;
   const void* couple;
   const void* macro;
@@ -461,7 +542,10 @@ KernelSet make_kernel_set(const char* name) {
   k.Q = Q; k.precision = (int)sizeof(T) * 8; k.collision = COLL; k.ddf = DDF; k.sensor = SENSOR;
   k.cells_per_thread = cells_per_thread<Q, T, COLL, DDF>;
   k.name = name;
-  k.sweep = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR>;
+  k.sweep = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, false>;
+  k.sweep_bricks = nullptr;
+  k.brick_cells_per_thread = sizeof(T) == 4 ? 2 : 1;
+  if constexpr (has_bricks<Q, T, COLL, DDF> && !SENSOR) k.sweep_bricks = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, true>;
   k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;
   k.couple = (const void*)&init_coupling_kernel<Q, T, COLL, DDF, SENSOR>;
   k.macro = (const void*)&macroscopic_kernel<Q, T, COLL, DDF>;

@@ -23,7 +23,7 @@ _ERR = {EINVAL: "LBM_EINVAL", ENOMEM: "LBM_ENOMEM", EMESH: "LBM_EMESH", ECUDA: "
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
-           "lbm_get_schedule", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_sync", "lbm_get_macroscopic",
+           "lbm_get_schedule", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_sync", "lbm_get_macroscopic",
            "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_measure_fma_peak"]
 
 
@@ -50,7 +50,7 @@ class LbmGridInfo(C.Structure):
         ("n_cells", C.c_int64 * MAX_LEVELS), ("n_inbox", C.c_int64 * MAX_LEVELS),
         ("n_coarse_ghosts", C.c_int64 * MAX_LEVELS), ("n_fine_ghosts", C.c_int64 * MAX_LEVELS),
         ("n_total", C.c_int64), ("updates_per_coarse_step", C.c_int64), ("launches_per_coarse_step", C.c_int64),
-        ("arena_bytes", C.c_size_t), ("tau", C.c_double * MAX_LEVELS),
+        ("arena_bytes", C.c_size_t), ("tau", C.c_double * MAX_LEVELS), ("n_bricks", C.c_int64 * MAX_LEVELS),
     ]
 
 
@@ -73,6 +73,7 @@ def lib():
         L.lbm_get_nbr.argtypes = [vp, C.c_int, vp]
         L.lbm_get_ghosts.argtypes = [vp, C.c_int, vp, vp, vp]
         L.lbm_get_schedule.argtypes = [vp, vp, vp, C.c_int]
+        L.lbm_get_bricks.argtypes = [vp, C.c_int, vp, vp]
         L.lbm_grid_bind.argtypes = [vp, vp, C.c_size_t, vp]
         L.lbm_init_fields.argtypes = [vp, vp, vp, vp, vp]
         L.lbm_step.argtypes = [vp, C.c_int]
@@ -180,6 +181,13 @@ class Grid:
         a = np.zeros((self.n[l], self.Q - 1), np.int32)
         _check("lbm_get_nbr", lib().lbm_get_nbr(self.h, l, _ptr(a)))
         return a
+
+    def bricks(self, l):
+        """(tiles9 [n_bricks, 9], table [Q-1, 64]) of lbm_get_bricks."""
+        nb = int(self.info.n_bricks[l])
+        t9 = np.zeros((nb, 9), np.int32); tab = np.zeros((self.Q - 1, 64), np.uint16)
+        _check("lbm_get_bricks", lib().lbm_get_bricks(self.h, l, _ptr(t9) if nb else None, _ptr(tab)))
+        return t9, tab
 
     def ghosts(self, l):
         ng = int(self.info.n_coarse_ghosts[l])

@@ -75,6 +75,61 @@ def test_host_builder_bit_exact_against_oracle_builder(name):
     g.close()
 
 
+def _zpos(m):
+    """(x, y) of Z-position m in an 8x8 tile, x in the even bits."""
+    x = (m & 1) | ((m >> 1) & 2) | ((m >> 2) & 4)
+    y = ((m >> 1) & 1) | ((m >> 2) & 2) | ((m >> 3) & 4)
+    return x, y
+
+
+@pytest.mark.parametrize("name", sorted(CASES))
+def test_bricks_reproduce_the_oracle_neighbour_list(name):
+    """Compressed addressing of the device path (lbm_get_bricks): every brick is an aligned 8x8 tile of FLUID cells
+    with consecutive storage indices, and tile arithmetic reproduces the ORACLE builder's neighbour list for each of
+    its cells and directions; the table itself is re-derived here from the lattice's velocities."""
+    case = CASES[name]()
+    g = lbm.Grid.from_case(case)
+    o = O.OracleGrid(O.make_config(**case.model_kwargs()), case.mesh.split, case.mesh.solid)
+    cx, cy, w, opp, cs2, reach = O.lattice(g.Q)
+    mm = np.arange(64)
+    for l in range(g.depth + 1):
+        t9, tab = g.bricks(l)
+        for i in range(1, g.Q):
+            for m in range(64):
+                x, y = _zpos(m)
+                sx, sy = x - cx[i], y - cy[i]
+                k = (0 if sx < 0 else 2 if sx > 7 else 1) + 3 * (0 if sy < 0 else 2 if sy > 7 else 1)
+                z = [mz for mz in range(64) if _zpos(mz) == (sx & 7, sy & 7)][0]
+                assert tab[i - 1, m] == (k << 6) | z
+        if len(t9) == 0:
+            continue
+        ix, iy, ty, aux = o.cells(l)
+        nbr = o.nbr(l)
+        base = t9[:, 4]
+        assert np.all(np.diff(base) >= 64)
+        cells = base[:, None] + mm[None, :]
+        assert np.all(ty[cells] == O.FLUID)
+        assert np.all(ix[base] % 8 == 0) and np.all(iy[base] % 8 == 0)
+        x, y = _zpos(mm)
+        assert np.array_equal(ix[cells], ix[base][:, None] + x[None, :])
+        assert np.array_equal(iy[cells], iy[base][:, None] + y[None, :])
+        for i in range(1, g.Q):
+            k, z = tab[i - 1] >> 6, tab[i - 1] & 63
+            assert np.array_equal(t9[:, k] + z[None, :], nbr[cells, i - 1])
+    g.close()
+
+
+def test_brick_coverage_of_the_bench_shapes():
+    """A periodic uniform box is all bricks; the graded cylinder mesh is mostly bricks on its fine levels."""
+    g = lbm.Grid.from_case(W.tgv(64))
+    assert int(g.info.n_bricks[0]) * 64 == g.n[0]
+    g.close()
+    g = lbm.Grid.from_case(W.cylinder(D=40))
+    frac = [int(g.info.n_bricks[l]) * 64 / g.n[l] for l in range(g.depth + 1)]
+    assert frac[0] > 0.8, frac
+    g.close()
+
+
 def test_invalid_arguments_are_rejected():
     with pytest.raises(lbm.LbmError) as e:
         lbm.Grid(lbm.make_config(lattice=10, nx_coarse=8, ny_coarse=8))
