@@ -64,6 +64,23 @@ def algorithmic_bytes_per_update(case, precision):
     return 2 * npop * (precision // 8) + (Q - 1) * 4 + 4
 
 
+def moved_bytes_per_update(g, case, precision):
+    """Bytes this implementation has to move per cell update, weighted over the levels by their share of the updates:
+    a cell of a regular brick needs its 2*npop reals and 36 B of tile bases per 64 cells; any
+    other cell the list row, the type byte and its entry of the irregular-cell list on top."""
+    Q = case.lattice
+    npop = Q * (2 if case.ddf else 1) + (8 if case.collision == W.NUMEQ else 0)
+    s = precision // 8
+    bricks = "bricks" in g.kernel_name()
+    tot = upd = 0.0
+    for l in range(g.depth + 1):
+        nb = 64 * int(g.info.n_bricks[l]) if bricks else 0
+        k = 1 << (g.depth - l)
+        tot += k * (nb * (2 * npop * s + 36.0 / 64) + (g.n[l] - nb) * (2 * npop * s + (Q - 1) * 4 + 1 + (4 if bricks else 0)))
+        upd += k * g.n[l]
+    return tot / upd
+
+
 def fine_equivalent_cells(case):
     m = case.mesh
     n = m.nx_coarse * m.ny_coarse * 4 ** m.depth
@@ -289,19 +306,30 @@ def main():
     K = args.steps
     mlups = aggregate_mlups(upd, K, world, ms)
     bpu = algorithmic_bytes_per_update(case, args.precision)
+    mbpu = moved_bytes_per_update(g, case, args.precision)
     peaks, peak_src = measured_peaks()
     peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
     achieved = upd * K * bpu / (ms * 1e-3) / 1e9          # this rank's kernel: all launches of the region are the sweep kernel
-    # dram bytes per launch of the dominant kernel (finest level's sweep) from the committed ncu --set full capture
+    # counters of the dominant kernel (finest level's sweep) from the committed ncu --set full captures
     traffic = traffic_src = None
+    counters = {}
     tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp) and args.scale == 1.0:
+    if os.path.exists(tp):
         try:
-            e = json.load(open(tp)).get("%s_f%d" % (args.workload, args.precision))
-            if e and int(e["cells_per_launch"]) == int(g.n[0]):
-                traffic, traffic_src = e["bytes_per_launch"], e["source"]
+            counters = json.load(open(tp)).get("%s_f%d" % (args.workload, args.precision)) or {}
+            if args.scale == 1.0 and int(counters.get("cells_per_launch", -1)) == int(g.n[0]):
+                traffic, traffic_src = counters["bytes_per_launch"], counters["source"]
         except Exception:
-            traffic = None
+            counters = {}
+    # ALU-bound path (numerical equilibria): fp64 flop per update from the ncu capture against the FMA peak measured now
+    alu = None
+    if case.collision == W.NUMEQ and "fp64_flop_per_update" in counters and args.precision == 64:
+        fma_peak, _ = lbm.measure_fma_peak(64, 1.0)
+        tf = upd * K * counters["fp64_flop_per_update"] / (ms * 1e-3) / 1e12
+        alu = {"bound": "alu", "achieved": tf, "peak": fma_peak, "unit": "TFLOP/s", "frac": tf / fma_peak, "traffic": traffic,
+               "peak_source": "lbm_measure_fma_peak(64) measured in this run (148 SMs x 64 fp64 FMA lanes x clock)",
+               "flop_per_update": counters["fp64_flop_per_update"], "flop_source": counters.get("fp64_note"),
+               "fp64_pipe_pct_ncu": counters.get("fp64_pipe_pct")}
     n_all = ntot
     depth = g.depth
     line = {
@@ -312,7 +340,7 @@ def main():
                        cells_per_level=g.n, updates_per_step=upd, step="one coarse step = %d fine steps" % (1 << depth),
                        parallelism="replicas x%d" % world, l2="inputs larger than L2 (state %.0f MB)" % (g.info.arena_bytes / 1e6)
                        if g.info.arena_bytes > 4 * 126e6 else "working set %.0f MB fits L2: launch-latency-bound case, no flush" % (g.info.arena_bytes / 1e6),
-                       kernel=g.kernel_name()),
+                       kernel=g.kernel_name(), brick_cell_share=[round(64 * int(g.info.n_bricks[l]) / max(g.n[l], 1), 4) for l in range(depth + 1)]),
         "mlups": {"actual": mlups, "paper_eq13": n_all * (1 << depth) * K * world / (ms * 1e-3) / 1e6,
                   "fine_equivalent": fine_equivalent_cells(case) * (1 << depth) * K * world / (ms * 1e-3) / 1e6},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
@@ -320,6 +348,9 @@ def main():
                      "algorithmic_bytes_per_launch": int(g.n[0]) * bpu, "kernel": "%s, finest level (%d cells per launch)" % (g.kernel_name(), g.n[0]),
                      "achieved_is": "algorithmic bytes of all level sweeps of the timed region / its CUDA-event time (every launch is this kernel)",
                      "peak_source": peak_src, "bytes_per_update": bpu,
+                     "moved_bytes_per_update": mbpu, "moved": achieved * mbpu / bpu, "frac_moved": achieved * mbpu / bpu / peak,
+                     "note": "achieved/frac use the list-addressed method's algorithmic bytes (SURVEY 8(d)); with regular bricks the kernel "
+                             "moves fewer bytes than that, so frac can exceed 1: moved/frac_moved count what this implementation must move",
                      "frac_of_nominal_8TBs": achieved / 8000.0},
         "burst": {"steps": kb, "ms_per_step": burst_ms, "value": upd / (burst_ms * 1e-3) / 1e6, "unit": "MLUPS (this rank)",
                   "roofline_frac": upd * bpu / (burst_ms * 1e-3) / 1e9 / peak,
@@ -331,6 +362,12 @@ def main():
         "clocks": clocks,
         "wall_s_timed_region": wall, "build_s": t_build,
     }
+    if alu is not None:       # the HBM view stays beside it
+        line["roofline_hbm"] = line["roofline"]
+        line["roofline"] = alu
+    elif "fp64_pipe_pct" in counters:
+        line["roofline"]["fp64_pipe_pct_ncu"] = counters["fp64_pipe_pct"]
+        line["roofline"]["fp64_tflops"] = upd * K * counters["fp64_flop_per_update"] / (ms * 1e-3) / 1e12
     if args.cpu_baseline_seconds > 0 and world >= 1:
         o = oracle_grid(case)
         v, nf, nu, dt = oracle_rate(o, args.cpu_baseline_seconds)

@@ -162,7 +162,8 @@ int lbm_set_populations(lbm_grid* g, int level, int which, const double* in);
 /* Device-time of the work enqueued by the last lbm_step call, in milliseconds (CUDA events recorded on
  * the bound stream around it); synchronises.  Negative error code on failure. */
 double lbm_last_step_ms(lbm_grid* g);
-/* Name of the compiled sweep kernel this grid dispatches to (static string), for profiles. */
+/* Name of the compiled sweep kernel this grid dispatches to (static string), for profiles; says whether the
+ * compressed addressing of regular bricks is in use (environment LBM_NO_BRICKS=1 at bind time turns it off). */
 const char* lbm_kernel_name(const lbm_grid* g);
 
 

@@ -536,7 +536,10 @@ double lbm_last_step_ms(lbm_grid* g) {
   return (double)ms;
 }
 
-const char* lbm_kernel_name(const lbm_grid* g) { return g ? g->ks->name : ""; }
+const char* lbm_kernel_name(const lbm_grid* g) {
+  if (!g) return "";
+  return (g->bound ? g->bricks : g->ks->sweep_bricks != nullptr) ? g->ks->bricks_name : g->ks->name;
+}
 
 int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double* T) {
   if (!g) return LBM_EINVAL;

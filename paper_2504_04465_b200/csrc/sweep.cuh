@@ -530,6 +530,7 @@ struct KernelSet {
   const char* name;
   const void* sweep;
   const void* sweep_bricks;   // same update with compressed addressing of regular bricks, or null
+  const char* bricks_name;
   int brick_cells_per_thread;
   const void* init;
   const void* couple;
@@ -537,13 +538,14 @@ struct KernelSet {
 };
 
 template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
-KernelSet make_kernel_set(const char* name) {
+KernelSet make_kernel_set(const char* name, const char* bricks_name) {
   KernelSet k;
   k.Q = Q; k.precision = (int)sizeof(T) * 8; k.collision = COLL; k.ddf = DDF; k.sensor = SENSOR;
   k.cells_per_thread = cells_per_thread<Q, T, COLL, DDF>;
   k.name = name;
   k.sweep = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, false>;
   k.sweep_bricks = nullptr;
+  k.bricks_name = bricks_name;
   k.brick_cells_per_thread = sizeof(T) == 4 ? 2 : 1;
   if constexpr (has_bricks<Q, T, COLL, DDF> && !SENSOR) k.sweep_bricks = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, true>;
   k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;
@@ -553,7 +555,8 @@ KernelSet make_kernel_set(const char* name) {
 }
 
 #define LBM_KSET(Q, T, COLL, DDF, SENSOR) \
-  make_kernel_set<Q, T, COLL, DDF, SENSOR>("sweep_kernel<" #Q "," #T "," #COLL "," #DDF "," #SENSOR ">")
+  make_kernel_set<Q, T, COLL, DDF, SENSOR>("sweep_kernel<" #Q "," #T "," #COLL "," #DDF "," #SENSOR ",false>", \
+                                           "sweep_kernel<" #Q "," #T "," #COLL "," #DDF "," #SENSOR ",true> (bricks + list)")
 
 // defined one per lattice (sweep_q*.cu) so that the instantiations compile in parallel
 int kernel_sets_q9(const KernelSet** out);
