@@ -147,7 +147,7 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   a.status = g->d_status;
   a.brick_nb = L.brick_nb; a.brick_tab = g->d_tab; a.irr = L.irr;
   a.nbrick = (int)L.nbrick; a.n_irr = (int)L.n_irr;
-  const int64_t cells_per_cta = (int64_t)BLOCK * g->ks->brick_cells_per_thread;
+  const int64_t cells_per_cta = g->ks->brick_cells_per_cta;
   a.brick_ctas = (int)((L.nbrick * 64 + cells_per_cta - 1) / cells_per_cta);
   int rc;
   if (g->bricks && L.nbrick > 0)

@@ -75,57 +75,81 @@ constexpr bool has_bricks = !DDF && COLL != LBM_NUMEQ && Q <= 21;
 // Regular-brick path: 64 consecutive cells = one aligned 8x8 tile of fluid cells whose pull sources are
 // base[tile k] + Z-position, (k, Z-position) from a 64-entry table per direction (computed
 // addressing in regular interiors).  Replaces (Q-1) x 4 B of list and the type byte per cell by 36 B per 64 cells.
+// A warp owns BRICK_UNITS_PER_WARP consecutive bricks (fp64: one 32-cell half of each, one cell per thread; fp32: all
+// 64 cells, two per thread): the 9 tile bases of a brick sit in lanes 0-8 of one coalesced load, issued together with
+// the table loads, and reach the other lanes by shuffle, so the index chain in front of the gathers is one load deep.
+// More than one brick per warp (table entries loaded once, next bases prefetched) was measured SLOWER (uniform fp64
+// 38.8 against 41.6 GLUPS, the 39 k-cell cavity halves): the bricks of a warp serialise and the grid shrinks.
+constexpr int BRICK_UNITS_PER_WARP = 1;
+
+template <typename T>
+constexpr int brick_cells_per_cta = 128 * (sizeof(T) == 4 ? 2 : 1) * BRICK_UNITS_PER_WARP;
+
 template <int Q, typename T, int COLL>
 __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelParams& p) {
   constexpr int CPT = sizeof(T) == 4 ? 2 : 1;
-  constexpr int BPC = 128 * CPT / 64;                       // bricks per CTA
-  const int lt = threadIdx.x * CPT;
-  const int brick = blockIdx.x * BPC + lt / 64;
-  if (brick >= a.nbrick) return;
-  const int m0 = lt % 64;
-  const int* __restrict__ nbk = a.brick_nb + 9ll * brick;
-  const int base = __ldg(nbk + 4);
+  constexpr int WPB = 64 / (32 * CPT);                       // warps per brick
+  constexpr int UPW = BRICK_UNITS_PER_WARP;
+  const int lane = threadIdx.x & 31;
+  const int wg = blockIdx.x * 4 + (threadIdx.x >> 5);        // warp index inside the brick part of the grid
+  const int part = wg % WPB;
+  const int brick0 = (wg / WPB) * UPW;                       // this warp: bricks brick0 .. brick0 + UPW - 1
+  if (brick0 >= a.nbrick) return;
+  const int m0 = part * 32 * CPT + lane * CPT;               // Z-position of this thread's first cell in every brick
   const long long ps = a.ps;
-  int src[CPT][Q];
+  unsigned e[CPT][(Q + 1) / 3];                               // three 10-bit table entries per register
 #pragma unroll
   for (int j = 0; j < CPT; ++j) {
-    src[j][0] = base + m0 + j;
+#pragma unroll
+    for (int w = 0; w < (Q + 1) / 3; ++w) e[j][w] = 0u;
     static_for<1, Q>([&](auto ic) {
       constexpr int I = decltype(ic)::value;
-      const int e = __ldg(a.brick_tab + (I - 1) * 64 + m0 + j);
-      src[j][I] = __ldg(nbk + (e >> 6)) + (e & 63);
+      e[j][(I - 1) / 3] |= (unsigned)__ldg(a.brick_tab + (I - 1) * 64 + m0 + j) << (10 * ((I - 1) % 3));
     });
   }
+  const int* __restrict__ nbk = a.brick_nb + 9ll * brick0;
+  int nbv = lane < 9 ? __ldg(nbk + lane) : 0;
   pdl_wait();
   const T* __restrict__ So = (const T*)a.So;
   T* __restrict__ Sn = (T*)a.Sn;
-  T f[CPT][Q], g[1][Q], lam[NLAMBDA];
+#pragma unroll 1
+  for (int k = 0; k < UPW && brick0 + k < a.nbrick; ++k) {
+    const int nbc = nbv;
+    if (k + 1 < UPW && brick0 + k + 1 < a.nbrick) nbv = lane < 9 ? __ldg(nbk + 9 * (k + 1) + lane) : 0;
+    const int base = __shfl_sync(0xffffffffu, nbc, 4);
+    T f[CPT][Q], g[1][Q], lam[NLAMBDA];
 #pragma unroll
-  for (int j = 0; j < CPT; ++j)
-    static_for<0, Q>([&](auto ic) {
-      constexpr int I = decltype(ic)::value;
-      f[j][I] = So[I * ps + src[j][I]];
-    });
-#pragma unroll
-  for (int j = 0; j < CPT; ++j) {
-    T rho;
-    collide<Q, T, COLL, false, false>(p, T(a.tau), f[j], g[0], lam, rho);
-    if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
-  }
-  // a brick starts at any storage index: CPT-wide stores when its first cell is CPT-aligned (uniform per brick)
-  if (CPT == 1 || base % CPT == 0) {
-#pragma unroll
-    for (int i = 0; i < Q; ++i) {
-      Vec<T, CPT> o;
-#pragma unroll
-      for (int j = 0; j < CPT; ++j) o.v[j] = f[j][i];
-      *reinterpret_cast<Vec<T, CPT>*>(Sn + i * ps + base + m0) = o;
+    for (int j = 0; j < CPT; ++j) {
+      f[j][0] = So[base + m0 + j];
+      static_for<1, Q>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        constexpr int SH = 10 * ((I - 1) % 3);
+        const unsigned ent = e[j][(I - 1) / 3];
+        const int src = __shfl_sync(0xffffffffu, nbc, (ent >> (SH + 6)) & 15u) + (int)((ent >> SH) & 63u);
+        f[j][I] = So[I * ps + src];
+      });
     }
-  } else {
 #pragma unroll
-    for (int i = 0; i < Q; ++i)
+    for (int j = 0; j < CPT; ++j) {
+      T rho;
+      collide<Q, T, COLL, false, false>(p, T(a.tau), f[j], g[0], lam, rho);
+      if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+    }
+    // a brick starts at any storage index: CPT-wide stores when its first cell is CPT-aligned (uniform per brick)
+    if (CPT == 1 || base % CPT == 0) {
 #pragma unroll
-      for (int j = 0; j < CPT; ++j) Sn[i * ps + base + m0 + j] = f[j][i];
+      for (int i = 0; i < Q; ++i) {
+        Vec<T, CPT> o;
+#pragma unroll
+        for (int j = 0; j < CPT; ++j) o.v[j] = f[j][i];
+        *reinterpret_cast<Vec<T, CPT>*>(Sn + i * ps + base + m0) = o;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < Q; ++i)
+#pragma unroll
+        for (int j = 0; j < CPT; ++j) Sn[i * ps + base + m0 + j] = f[j][i];
+    }
   }
 }
 
@@ -531,7 +555,7 @@ struct KernelSet {
   const void* sweep;
   const void* sweep_bricks;   // same update with compressed addressing of regular bricks, or null
   const char* bricks_name;
-  int brick_cells_per_thread;
+  int brick_cells_per_cta;
   const void* init;
   const void* couple;
   const void* macro;
@@ -546,7 +570,7 @@ KernelSet make_kernel_set(const char* name, const char* bricks_name) {
   k.sweep = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, false>;
   k.sweep_bricks = nullptr;
   k.bricks_name = bricks_name;
-  k.brick_cells_per_thread = sizeof(T) == 4 ? 2 : 1;
+  k.brick_cells_per_cta = brick_cells_per_cta<T>;
   if constexpr (has_bricks<Q, T, COLL, DDF> && !SENSOR) k.sweep_bricks = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, true>;
   k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;
   k.couple = (const void*)&init_coupling_kernel<Q, T, COLL, DDF, SENSOR>;
