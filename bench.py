@@ -74,7 +74,7 @@ def moved_bytes_per_update(g, case, precision):
     bricks = "bricks" in g.kernel_name()
     tot = upd = 0.0
     for l in range(g.depth + 1):
-        nb = 64 * int(g.info.n_bricks[l]) if bricks else 0
+        nb = 64 * int(g.info.n_bricks[l]) if bricks and g.n[l] >= int(g.info.brick_min_level_cells) else 0
         k = 1 << (g.depth - l)
         tot += k * (nb * (2 * npop * s + 36.0 / 64) + (g.n[l] - nb) * (2 * npop * s + (Q - 1) * 4 + 1 + (4 if bricks else 0)))
         upd += k * g.n[l]
@@ -340,7 +340,8 @@ def main():
                        cells_per_level=g.n, updates_per_step=upd, step="one coarse step = %d fine steps" % (1 << depth),
                        parallelism="replicas x%d" % world, l2="inputs larger than L2 (state %.0f MB)" % (g.info.arena_bytes / 1e6)
                        if g.info.arena_bytes > 4 * 126e6 else "working set %.0f MB fits L2: launch-latency-bound case, no flush" % (g.info.arena_bytes / 1e6),
-                       kernel=g.kernel_name(), brick_cell_share=[round(64 * int(g.info.n_bricks[l]) / max(g.n[l], 1), 4) for l in range(depth + 1)]),
+                       kernel=g.kernel_name(), brick_cell_share=[round(64 * int(g.info.n_bricks[l]) / max(g.n[l], 1), 4) if g.n[l] >= int(g.info.brick_min_level_cells) else 0.0
+                                         for l in range(depth + 1)]),
         "mlups": {"actual": mlups, "paper_eq13": n_all * (1 << depth) * K * world / (ms * 1e-3) / 1e6,
                   "fine_equivalent": fine_equivalent_cells(case) * (1 << depth) * K * world / (ms * 1e-3) / 1e6},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

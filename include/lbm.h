@@ -89,6 +89,7 @@ typedef struct {
   size_t  arena_bytes;                    /* device memory the caller must provide to lbm_grid_bind */
   double  tau[LBM_MAX_LEVELS];
   int64_t n_bricks[LBM_MAX_LEVELS];       /* regular 8x8 bricks (64 cells each) addressed by tile arithmetic on the device */
+  int64_t brick_min_level_cells;          /* levels with fewer stored cells go through the list (latency-bound) */
 } lbm_grid_info;
 
 typedef struct lbm_grid lbm_grid;   /* opaque */

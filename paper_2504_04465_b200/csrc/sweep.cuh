@@ -75,29 +75,29 @@ constexpr bool has_bricks = !DDF && COLL != LBM_NUMEQ && Q <= 21;
 // Regular-brick path: 64 consecutive cells = one aligned 8x8 tile of fluid cells whose pull sources are
 // base[tile k] + Z-position, (k, Z-position) from a 64-entry table per direction (computed
 // addressing in regular interiors).  Replaces (Q-1) x 4 B of list and the type byte per cell by 36 B per 64 cells.
-// A warp owns BRICK_UNITS_PER_WARP consecutive bricks (fp64: one 32-cell half of each, one cell per thread; fp32: all
-// 64 cells, two per thread): the 9 tile bases of a brick sit in lanes 0-8 of one coalesced load, issued together with
-// the table loads, and reach the other lanes by shuffle, so the index chain in front of the gathers is one load deep.
-// More than one brick per warp (table entries loaded once, next bases prefetched) was measured SLOWER (uniform fp64
-// 38.8 against 41.6 GLUPS, the 39 k-cell cavity halves): the bricks of a warp serialise and the grid shrinks.
-constexpr int BRICK_UNITS_PER_WARP = 1;
-
-template <typename T>
-constexpr int brick_cells_per_cta = 128 * (sizeof(T) == 4 ? 2 : 1) * BRICK_UNITS_PER_WARP;
+// A thread owns BRICK_CPT = 2 consecutive cells (an x-adjacent pair; 128-bit stores in fp64, 64-bit in fp32), so a
+// brick is one warp (measured: fp64 1 -> 2 cells per thread +7 %; fp32 2 -> 4 cells per thread -3 %, the grid shrinks).  The 9 tile bases of a brick sit in the first 9 lanes of its thread group (one coalesced load, issued
+// together with the table loads) and reach the other lanes by shuffle, so the index chain in front of the gathers is
+// one load deep and there is no per-cell index traffic.
+// (Several bricks per warp in sequence, with the table entries loaded once and the next bases prefetched, was measured
+// SLOWER: uniform fp64 38.8 against 41.6 GLUPS, the 39 k-cell cavity halves -- the bricks serialise and the grid shrinks.)
+template <typename T> constexpr int BRICK_CPT = 2;
+template <typename T> constexpr int brick_cells_per_cta = 128 * BRICK_CPT<T>;
 
 template <int Q, typename T, int COLL>
 __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelParams& p) {
-  constexpr int CPT = sizeof(T) == 4 ? 2 : 1;
-  constexpr int WPB = 64 / (32 * CPT);                       // warps per brick
-  constexpr int UPW = BRICK_UNITS_PER_WARP;
+  constexpr int CPT = BRICK_CPT<T>;
+  constexpr int TPB = 64 / CPT;                              // threads per brick
   const int lane = threadIdx.x & 31;
-  const int wg = blockIdx.x * 4 + (threadIdx.x >> 5);        // warp index inside the brick part of the grid
-  const int part = wg % WPB;
-  const int brick0 = (wg / WPB) * UPW;                       // this warp: bricks brick0 .. brick0 + UPW - 1
-  if (brick0 >= a.nbrick) return;
-  const int m0 = part * 32 * CPT + lane * CPT;               // Z-position of this thread's first cell in every brick
+  const int sub = lane % TPB;                                // thread index inside its brick
+  const int grp = lane - sub;                                // first lane of the brick's thread group
+  const int brick_raw = (blockIdx.x * 128 + threadIdx.x) / TPB;
+  if (brick_raw - (lane / TPB) >= a.nbrick) return;          // whole warp beyond the last brick
+  const bool valid = brick_raw < a.nbrick;                   // (a trailing thread group recomputes the last brick, unstored)
+  const int brick = valid ? brick_raw : a.nbrick - 1;
+  const int m0 = sub * CPT;                                  // Z-position of this thread's first cell
   const long long ps = a.ps;
-  unsigned e[CPT][(Q + 1) / 3];                               // three 10-bit table entries per register
+  unsigned e[CPT][(Q + 1) / 3];                              // three 10-bit table entries per register
 #pragma unroll
   for (int j = 0; j < CPT; ++j) {
 #pragma unroll
@@ -107,49 +107,44 @@ __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelPara
       e[j][(I - 1) / 3] |= (unsigned)__ldg(a.brick_tab + (I - 1) * 64 + m0 + j) << (10 * ((I - 1) % 3));
     });
   }
-  const int* __restrict__ nbk = a.brick_nb + 9ll * brick0;
-  int nbv = lane < 9 ? __ldg(nbk + lane) : 0;
+  const int nbv = sub < 9 ? __ldg(a.brick_nb + 9ll * brick + sub) : 0;
   pdl_wait();
   const T* __restrict__ So = (const T*)a.So;
   T* __restrict__ Sn = (T*)a.Sn;
-#pragma unroll 1
-  for (int k = 0; k < UPW && brick0 + k < a.nbrick; ++k) {
-    const int nbc = nbv;
-    if (k + 1 < UPW && brick0 + k + 1 < a.nbrick) nbv = lane < 9 ? __ldg(nbk + 9 * (k + 1) + lane) : 0;
-    const int base = __shfl_sync(0xffffffffu, nbc, 4);
-    T f[CPT][Q], g[1][Q], lam[NLAMBDA];
+  const int base = __shfl_sync(0xffffffffu, nbv, grp + 4);
+  T f[CPT][Q], g[1][Q], lam[NLAMBDA];
 #pragma unroll
-    for (int j = 0; j < CPT; ++j) {
-      f[j][0] = So[base + m0 + j];
-      static_for<1, Q>([&](auto ic) {
-        constexpr int I = decltype(ic)::value;
-        constexpr int SH = 10 * ((I - 1) % 3);
-        const unsigned ent = e[j][(I - 1) / 3];
-        const int src = __shfl_sync(0xffffffffu, nbc, (ent >> (SH + 6)) & 15u) + (int)((ent >> SH) & 63u);
-        f[j][I] = So[I * ps + src];
-      });
+  for (int j = 0; j < CPT; ++j) {
+    f[j][0] = So[base + m0 + j];
+    static_for<1, Q>([&](auto ic) {
+      constexpr int I = decltype(ic)::value;
+      constexpr int SH = 10 * ((I - 1) % 3);
+      const unsigned ent = e[j][(I - 1) / 3];
+      const int src = __shfl_sync(0xffffffffu, nbv, grp + (int)((ent >> (SH + 6)) & 15u)) + (int)((ent >> SH) & 63u);
+      f[j][I] = So[I * ps + src];
+    });
+  }
+#pragma unroll
+  for (int j = 0; j < CPT; ++j) {
+    T rho;
+    collide<Q, T, COLL, false, false>(p, T(a.tau), f[j], g[0], lam, rho);
+    if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
+  }
+  if (!valid) return;
+  // a brick starts at any storage index: 128-bit stores when its first cell is CPT-aligned (uniform per brick)
+  if (base % CPT == 0) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+      Vec<T, CPT> o;
+#pragma unroll
+      for (int j = 0; j < CPT; ++j) o.v[j] = f[j][i];
+      *reinterpret_cast<Vec<T, CPT>*>(Sn + i * ps + base + m0) = o;
     }
+  } else {
 #pragma unroll
-    for (int j = 0; j < CPT; ++j) {
-      T rho;
-      collide<Q, T, COLL, false, false>(p, T(a.tau), f[j], g[0], lam, rho);
-      if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
-    }
-    // a brick starts at any storage index: CPT-wide stores when its first cell is CPT-aligned (uniform per brick)
-    if (CPT == 1 || base % CPT == 0) {
+    for (int i = 0; i < Q; ++i)
 #pragma unroll
-      for (int i = 0; i < Q; ++i) {
-        Vec<T, CPT> o;
-#pragma unroll
-        for (int j = 0; j < CPT; ++j) o.v[j] = f[j][i];
-        *reinterpret_cast<Vec<T, CPT>*>(Sn + i * ps + base + m0) = o;
-      }
-    } else {
-#pragma unroll
-      for (int i = 0; i < Q; ++i)
-#pragma unroll
-        for (int j = 0; j < CPT; ++j) Sn[i * ps + base + m0 + j] = f[j][i];
-    }
+      for (int j = 0; j < CPT; ++j) Sn[i * ps + base + m0 + j] = f[j][i];
   }
 }
 
@@ -168,7 +163,7 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
     }
     const int t = ((int)blockIdx.x - a.brick_ctas) * blockDim.x + threadIdx.x;
     if (t >= a.n_irr) return;
-    c0 = a.irr[t];
+    c0 = a.irr ? a.irr[t] : t;              // irr == null: every cell of a small level through the list, one per thread
   } else {
     c0 = (blockIdx.x * blockDim.x + threadIdx.x) * CPT;
     if (c0 >= a.n) return;

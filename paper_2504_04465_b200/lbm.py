@@ -51,6 +51,7 @@ class LbmGridInfo(C.Structure):
         ("n_coarse_ghosts", C.c_int64 * MAX_LEVELS), ("n_fine_ghosts", C.c_int64 * MAX_LEVELS),
         ("n_total", C.c_int64), ("updates_per_coarse_step", C.c_int64), ("launches_per_coarse_step", C.c_int64),
         ("arena_bytes", C.c_size_t), ("tau", C.c_double * MAX_LEVELS), ("n_bricks", C.c_int64 * MAX_LEVELS),
+        ("brick_min_level_cells", C.c_int64),
     ]
 
 
