@@ -68,33 +68,35 @@ template <typename T, int N> struct alignas(sizeof(T) * N) Vec { T v[N]; };
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-// Models whose regular interior is updated through bricks (weakly compressible, one population set).
+// Models whose regular interior is updated through bricks: the polynomial ones (the numerical-equilibrium kernels are
+// fp64-ALU-bound, their list is 9 % of the traffic and their registers are spoken for).
 template <int Q, typename T, int COLL, bool DDF>
-constexpr bool has_bricks = !DDF && COLL != LBM_NUMEQ && Q <= 21;
+constexpr bool has_bricks = COLL != LBM_NUMEQ;
 
 // Regular-brick path: 64 consecutive cells = one aligned 8x8 tile of fluid cells whose pull sources are
 // base[tile k] + Z-position, (k, Z-position) from a 64-entry table per direction (computed
 // addressing in regular interiors).  Replaces (Q-1) x 4 B of list and the type byte per cell by 36 B per 64 cells.
-// A thread owns BRICK_CPT = 2 consecutive cells (an x-adjacent pair; 128-bit stores in fp64, 64-bit in fp32), so a
-// brick is one warp (measured: fp64 1 -> 2 cells per thread +7 %; fp32 2 -> 4 cells per thread -3 %, the grid shrinks).  The 9 tile bases of a brick sit in the first 9 lanes of its thread group (one coalesced load, issued
+// D2Q9/13: a thread owns 2 consecutive cells (an x-adjacent pair; 128-bit stores in fp64, 64-bit in fp32), so a brick
+// is one warp (measured: fp64 1 -> 2 cells per thread +7 %; fp32 2 -> 4 cells per thread -3 %, the grid shrinks); the
+// wide models (D2Q21/37, second distribution) keep one cell per thread (registers), a brick is two warps.  The 9 tile bases of a brick sit in the first 9 lanes of its thread group (one coalesced load, issued
 // together with the table loads) and reach the other lanes by shuffle, so the index chain in front of the gathers is
 // one load deep and there is no per-cell index traffic.
 // (Several bricks per warp in sequence, with the table entries loaded once and the next bases prefetched, was measured
 // SLOWER: uniform fp64 38.8 against 41.6 GLUPS, the 39 k-cell cavity halves -- the bricks serialise and the grid shrinks.)
-template <typename T> constexpr int BRICK_CPT = 2;
-template <typename T> constexpr int brick_cells_per_cta = 128 * BRICK_CPT<T>;
+template <int Q, bool DDF> constexpr int BRICK_CPT = (Q <= 13 && !DDF) ? 2 : 1;
+template <int Q, bool DDF> constexpr int brick_cells_per_cta = 128 * BRICK_CPT<Q, DDF>;
 
-template <int Q, typename T, int COLL>
+template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
 __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelParams& p) {
-  constexpr int CPT = BRICK_CPT<T>;
-  constexpr int TPB = 64 / CPT;                              // threads per brick
+  using PL = PopLayout<Q, DDF, COLL>;
+  constexpr int CPT = BRICK_CPT<Q, DDF>;
+  constexpr int TPB = 64 / CPT;                              // threads per brick: 32 or 64 (a brick never shares a warp)
   const int lane = threadIdx.x & 31;
-  const int sub = lane % TPB;                                // thread index inside its brick
-  const int grp = lane - sub;                                // first lane of the brick's thread group
+  const int sub = threadIdx.x % TPB;                         // thread index inside its brick
+  constexpr int grp = 0;                                     // lanes 0-8 of every warp hold the tile bases
   const int brick_raw = (blockIdx.x * 128 + threadIdx.x) / TPB;
-  if (brick_raw - (lane / TPB) >= a.nbrick) return;          // whole warp beyond the last brick
-  const bool valid = brick_raw < a.nbrick;                   // (a trailing thread group recomputes the last brick, unstored)
-  const int brick = valid ? brick_raw : a.nbrick - 1;
+  if (brick_raw >= a.nbrick) return;                         // whole warp beyond the last brick
+  const int brick = brick_raw;
   const int m0 = sub * CPT;                                  // Z-position of this thread's first cell
   const long long ps = a.ps;
   unsigned e[CPT][(Q + 1) / 3];                              // three 10-bit table entries per register
@@ -107,30 +109,31 @@ __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelPara
       e[j][(I - 1) / 3] |= (unsigned)__ldg(a.brick_tab + (I - 1) * 64 + m0 + j) << (10 * ((I - 1) % 3));
     });
   }
-  const int nbv = sub < 9 ? __ldg(a.brick_nb + 9ll * brick + sub) : 0;
+  const int nbv = lane < 9 ? __ldg(a.brick_nb + 9ll * brick + lane) : 0;
   pdl_wait();
   const T* __restrict__ So = (const T*)a.So;
   T* __restrict__ Sn = (T*)a.Sn;
   const int base = __shfl_sync(0xffffffffu, nbv, grp + 4);
-  T f[CPT][Q], g[1][Q], lam[NLAMBDA];
+  T f[CPT][Q], g[CPT][Q], lam[NLAMBDA];
 #pragma unroll
   for (int j = 0; j < CPT; ++j) {
     f[j][0] = So[base + m0 + j];
+    if constexpr (DDF) g[j][0] = So[PL::G0 * ps + base + m0 + j];
     static_for<1, Q>([&](auto ic) {
       constexpr int I = decltype(ic)::value;
       constexpr int SH = 10 * ((I - 1) % 3);
       const unsigned ent = e[j][(I - 1) / 3];
       const int src = __shfl_sync(0xffffffffu, nbv, grp + (int)((ent >> (SH + 6)) & 15u)) + (int)((ent >> SH) & 63u);
       f[j][I] = So[I * ps + src];
+      if constexpr (DDF) g[j][I] = So[(PL::G0 + I) * ps + src];
     });
   }
 #pragma unroll
   for (int j = 0; j < CPT; ++j) {
     T rho;
-    collide<Q, T, COLL, false, false>(p, T(a.tau), f[j], g[0], lam, rho);
+    collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f[j], g[j], lam, rho);
     if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
   }
-  if (!valid) return;
   // a brick starts at any storage index: 128-bit stores when its first cell is CPT-aligned (uniform per brick)
   if (base % CPT == 0) {
 #pragma unroll
@@ -139,12 +142,20 @@ __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelPara
 #pragma unroll
       for (int j = 0; j < CPT; ++j) o.v[j] = f[j][i];
       *reinterpret_cast<Vec<T, CPT>*>(Sn + i * ps + base + m0) = o;
+      if constexpr (DDF) {
+#pragma unroll
+        for (int j = 0; j < CPT; ++j) o.v[j] = g[j][i];
+        *reinterpret_cast<Vec<T, CPT>*>(Sn + (PL::G0 + i) * ps + base + m0) = o;
+      }
     }
   } else {
 #pragma unroll
     for (int i = 0; i < Q; ++i)
 #pragma unroll
-      for (int j = 0; j < CPT; ++j) Sn[i * ps + base + m0 + j] = f[j][i];
+      for (int j = 0; j < CPT; ++j) {
+        Sn[i * ps + base + m0 + j] = f[j][i];
+        if constexpr (DDF) Sn[(PL::G0 + i) * ps + base + m0 + j] = g[j][i];
+      }
   }
 }
 
@@ -156,9 +167,9 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
   pdl_launch_dependents();
   int c0;
   if constexpr (BRICKS) {
-    static_assert(has_bricks<Q, T, COLL, DDF> && !SENSOR, "no brick path for this model");
+    static_assert(has_bricks<Q, T, COLL, DDF>, "no brick path for this model");
     if ((int)blockIdx.x < a.brick_ctas) {
-      brick_update<Q, T, COLL>(a, p);
+      brick_update<Q, T, COLL, DDF, SENSOR>(a, p);
       return;
     }
     const int t = ((int)blockIdx.x - a.brick_ctas) * blockDim.x + threadIdx.x;
@@ -565,8 +576,8 @@ KernelSet make_kernel_set(const char* name, const char* bricks_name) {
   k.sweep = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, false>;
   k.sweep_bricks = nullptr;
   k.bricks_name = bricks_name;
-  k.brick_cells_per_cta = brick_cells_per_cta<T>;
-  if constexpr (has_bricks<Q, T, COLL, DDF> && !SENSOR) k.sweep_bricks = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, true>;
+  k.brick_cells_per_cta = brick_cells_per_cta<Q, DDF>;
+  if constexpr (has_bricks<Q, T, COLL, DDF>) k.sweep_bricks = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, true>;
   k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;
   k.couple = (const void*)&init_coupling_kernel<Q, T, COLL, DDF, SENSOR>;
   k.macro = (const void*)&macroscopic_kernel<Q, T, COLL, DDF>;
