@@ -123,9 +123,10 @@ __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelPara
       constexpr int I = decltype(ic)::value;
       constexpr int SH = 10 * ((I - 1) % 3);
       const unsigned ent = e[j][(I - 1) / 3];
-      const int src = __shfl_sync(0xffffffffu, nbv, grp + (int)((ent >> (SH + 6)) & 15u)) + (int)((ent >> SH) & 63u);
-      f[j][I] = So[I * ps + src];
-      if constexpr (DDF) g[j][I] = So[(PL::G0 + I) * ps + src];
+      // unsigned 32-bit cell index against a warp-uniform plane pointer: one address instruction per gather
+      const unsigned src = (unsigned)__shfl_sync(0xffffffffu, nbv, grp + (int)((ent >> (SH + 6)) & 15u)) + ((ent >> SH) & 63u);
+      f[j][I] = (So + I * ps)[src];
+      if constexpr (DDF) g[j][I] = (So + (PL::G0 + I) * ps)[src];
     });
   }
 #pragma unroll
