@@ -33,6 +33,11 @@ if ROOT not in sys.path:
 
 from paper_2504_04465_b200 import workloads as W   # input generators only (no arithmetic of the method)
 
+# Table 3a: A100-SXM4-80GB, single precision, MLUPS of Eq. 13 (all cells x finest iterations), L = 2^13
+# (D2Q37 unif: 2^12).  Context for vs_baseline of `--workload sod:<lattice>:<mesh> --precision 32`.
+PAPER_TABLE3 = {(13, "unif"): 1259.1, (13, "hori"): 1088.4, (13, "band"): 1244.8, (13, "sqr"): 1072.7,
+                (21, "unif"): 618.5, (21, "hori"): 555.9, (21, "band"): 588.2, (21, "sqr"): 544.4,
+                (37, "unif"): 286.9, (37, "hori"): 263.0, (37, "band"): 307.4, (37, "sqr"): 266.1}
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 
 
@@ -53,6 +58,15 @@ def make_case(name, scale):
     if name == "naca":
         c = int(round(1024 * scale))
         return W.naca(chord=c), dict(workload="naca (BASELINE configs[4]): D2Q21 numerical eq.+g+sensor, chord %d, 7 levels" % c, steps=8)
+    if name.startswith("sod"):
+        # sod[:lattice[:mesh]], e.g. sod:21:unif -- the paper's only absolute GPU figures (Table 3a)
+        parts = name.split(":")
+        lat = int(parts[1]) if len(parts) > 1 else 21
+        mesh = parts[2] if len(parts) > 2 else "unif"
+        L = int(round((4096 if (lat == 37 and mesh == "unif") else 8192) * scale))
+        return W.sod(L=L, lattice=lat, mesh=mesh), dict(
+            workload="sod shock tube (Table 3, P:656): D2Q%d numerical eq.+g+sensor, mesh %s, L=%d, periodic box" % (lat, mesh, L),
+            steps=100, paper_mlups=PAPER_TABLE3.get((lat, mesh)))
     raise SystemExit("unknown workload %r" % name)
 
 
@@ -332,9 +346,14 @@ def main():
                "fp64_pipe_pct_ncu": counters.get("fp64_pipe_pct")}
     n_all = ntot
     depth = g.depth
+    # vs_baseline only where BASELINE.md holds the paper's number for this exact metric and workload: Table 3a, Eq. 13
+    # MLUPS, single precision, full size (another machine's figure: context, not the target)
+    vs_baseline = None
+    if info.get("paper_mlups") and args.precision == 32 and args.scale == 1.0 and world == 1:
+        vs_baseline = n_all * (1 << depth) * K / (ms * 1e-3) / 1e6 / info["paper_mlups"]
     line = {
         "metric": "MLUPS (actual cell updates per second)", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K,
-        "warmup": args.warmup, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "warmup": args.warmup, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": vs_baseline,
         "dtype": "f%d" % args.precision, "data": "synthetic",
         "config": dict(workload=info["workload"], precision=args.precision, cells=n_all, levels=depth + 1,
                        cells_per_level=g.n, updates_per_step=upd, step="one coarse step = %d fine steps" % (1 << depth),

@@ -157,7 +157,10 @@ class Grid:
 
     @classmethod
     def from_case(cls, case, precision=64):
-        return cls(make_config(precision=precision, **case.model_kwargs()), case.mesh.split, case.mesh.solid)
+        kw = case.model_kwargs()
+        if precision == 32:      # Newton tolerance of single-precision runs (1e-12 in fp64, 1e-5 in fp32)
+            kw["newton_tol"] = max(kw["newton_tol"], 1e-5)
+        return cls(make_config(precision=precision, **kw), case.mesh.split, case.mesh.solid)
 
     def close(self):
         if getattr(self, "h", None):

@@ -220,6 +220,43 @@ def riemann(n=2048, seed=7, lattice=37, periodic=False, sensor=1, tau0=0.5, gamm
                 meta=dict(n=n, rho=rho_q, T=T_q, ux=ux_q, uy=uy_q))
 
 
+# ----------------------------------------------------------------------------- Sod shock tube
+SOD_T0 = {13: 0.35, 21: 0.9, 37: 1.0}      # inviscid reference temperatures
+
+
+def sod(L=8192, lattice=21, mesh="unif", periodic=True, sensor_A=1.5, gamma=1.4, ny=None):
+    """Inviscid Sod shock tube (Eq. 12: (p, rho, u) = (10, 8, 0) p0, rho0 left of x = L/2, (1, 1, 0) right) on an
+    L x L box (L = finest-equivalent cells per side) with numerical equilibria + g + sensor (A = 1.5), tau = 1/2
+    (P:940).  Meshes of Sec. 6.1 / Table 3: unif; hori (fine below y = L/2), band (fine for
+    L/4 <= x < 3L/4), sqr (fine L/2 square at the centre), each two levels over a coarse L/2 x L/2 box.
+    periodic=True (throughput runs): fully periodic box, i.e. a second, mirrored Riemann problem at the seam x = 0;
+    periodic=False (physics pin, unif only): Neumann ends in x, periodic in y; ny: height of the unif box (default L)."""
+    T0 = SOD_T0[lattice]
+    rho_r, T_r = 1.0, T0                     # right state: rho0 = 1, p0 = rho0 T0
+    rho_l, T_l = 8.0, 10.0 / 8.0 * T0        # p = 10 p0, rho = 8 rho0
+
+    def fields(level, ix, iy):
+        x, _ = centres(level, ix, iy)
+        left = x < 0.5 * L
+        z = np.zeros(len(x))
+        return np.where(left, rho_l, rho_r), z, z, np.where(left, T_l, T_r)
+
+    if mesh == "unif":
+        m = uniform_mesh(L, L if ny is None else ny)
+    else:
+        nc = L // 2
+        assert 2 * nc == L and mesh in ("hori", "band", "sqr"), mesh
+
+        def refine(level, ix, iy):
+            inx = (ix >= nc // 4) & (ix < 3 * nc // 4)
+            iny = (iy >= nc // 4) & (iy < 3 * nc // 4)
+            return {"hori": iy < nc // 2, "band": inx, "sqr": inx & iny}[mesh]
+        m = build_mesh(1, nc, nc, refine)
+    bc = (BC_PERIODIC,) * 4 if periodic else (BC_NEUMANN, BC_NEUMANN, BC_PERIODIC, BC_PERIODIC)
+    return Case("sod", m, lattice=lattice, collision=NUMEQ, ddf=1, sensor=1, tau0=0.5, T0=T0, gamma=gamma, sensor_A=sensor_A,
+                bc=bc, fields=fields, meta=dict(L=L, mesh=mesh, left=(rho_l, 0.0, T_l), right=(rho_r, 0.0, T_r)))
+
+
 # ----------------------------------------------------------------------------- config 5
 NACA_RADII_C = (1.0, 2.25, 5.0, 9.0, 12.5, 14.0)   # R_0..R_5 in chords (DESIGN.md)
 

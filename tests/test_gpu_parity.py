@@ -210,3 +210,22 @@ def test_unstable_state_is_reported():
     g.step(1)
     assert g.sync() == lbm.EUNSTABLE
     g.close()
+
+
+# ------------------------------------------------------------------ Sod shock tube (Table 3)
+@pytest.mark.parametrize("lattice", [13, 21, 37])
+@pytest.mark.parametrize("mesh", ["unif", "band", "sqr", "hori"])
+def test_sod_numerical_equilibrium_fp64_and_fp32(lattice, mesh):
+    """Numerical equilibria + g + sensor on the paper's four Sod meshes, fp64 (|df| <= 1e-12) and fp32 with the
+    single-precision Newton tolerance of P:934 (|df| <= 1e-5) against the fp64 oracle."""
+    case = W.sod(L=64, lattice=lattice, mesh=mesh)
+    o = oracle_from_case(case)
+    ncoarse = 3
+    assert o.step(ncoarse) == 0
+    for prec, tol in ((64, 1e-12), (32, 1e-5)):
+        g = gpu_from_case(case, prec)
+        g.step(ncoarse)
+        assert g.sync() == 0
+        d = max_pop_diff(g, o, (0, 1))
+        assert d <= tol * 8.0, (lattice, mesh, prec, d)      # populations scale with rho <= 8 (Eq. 12)
+        g.close()
