@@ -12,6 +12,9 @@
 //   DIRICHLET         stores the equilibrium of the imposed state.
 // Each thread writes only its own slot (and its own children), so there are no atomics and no
 // write hazards; the two-buffer scheme of the paper is kept.
+// BRICKS kernels put a second addressing in front of that list path: regular 8x8 tiles of fluid cells ("bricks",
+// verified against the list by the host builder) are updated by the first CTAs of the same launch through tile
+// arithmetic, without list, type or link handling (brick_update below).
 #pragma once
 #include "collide.cuh"
 
@@ -76,20 +79,21 @@ constexpr bool has_bricks = COLL != LBM_NUMEQ;
 // Regular-brick path: 64 consecutive cells = one aligned 8x8 tile of fluid cells whose pull sources are
 // base[tile k] + Z-position, (k, Z-position) from a 64-entry table per direction (computed
 // addressing in regular interiors).  Replaces (Q-1) x 4 B of list and the type byte per cell by 36 B per 64 cells.
-// D2Q9/13: a thread owns 2 consecutive cells (an x-adjacent pair; 128-bit stores in fp64, 64-bit in fp32), so a brick
-// is one warp (measured: fp64 1 -> 2 cells per thread +7 %; fp32 2 -> 4 cells per thread -3 %, the grid shrinks); the
-// wide models (D2Q21/37, second distribution) keep one cell per thread (registers), a brick is two warps.  The 9 tile bases of a brick sit in the first 9 lanes of its thread group (one coalesced load, issued
-// together with the table loads) and reach the other lanes by shuffle, so the index chain in front of the gathers is
-// one load deep and there is no per-cell index traffic.
+// Cells of up to 104 bytes of populations (D2Q9/13 in fp64, D2Q9/13/21 in fp32): a thread owns 2 consecutive cells
+// (an x-adjacent pair; 128-bit stores in fp64, 64-bit in fp32), so a brick is one warp (measured: fp64 1 -> 2 cells
+// per thread +7 %; fp32 2 -> 4 cells per thread -3 %, the grid shrinks).  Wider cells (D2Q21 fp64, D2Q37, second
+// distribution) keep one cell per thread (registers); a brick is then two warps.  The 9 tile bases of a brick sit in
+// lanes 0-8 of each of its warps (one coalesced load, issued together with the table loads) and reach the other lanes
+// by shuffle, so the index chain in front of the gathers is one load deep and there is no per-cell index traffic.
 // (Several bricks per warp in sequence, with the table entries loaded once and the next bases prefetched, was measured
 // SLOWER: uniform fp64 38.8 against 41.6 GLUPS, the 39 k-cell cavity halves -- the bricks serialise and the grid shrinks.)
-template <int Q, bool DDF> constexpr int BRICK_CPT = (Q <= 13 && !DDF) ? 2 : 1;
-template <int Q, bool DDF> constexpr int brick_cells_per_cta = 128 * BRICK_CPT<Q, DDF>;
+template <int Q, typename T, bool DDF> constexpr int BRICK_CPT = (Q * (DDF ? 2 : 1) * (int)sizeof(T) <= 104) ? 2 : 1;
+template <int Q, typename T, bool DDF> constexpr int brick_cells_per_cta = 128 * BRICK_CPT<Q, T, DDF>;
 
 template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
 __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelParams& p) {
   using PL = PopLayout<Q, DDF, COLL>;
-  constexpr int CPT = BRICK_CPT<Q, DDF>;
+  constexpr int CPT = BRICK_CPT<Q, T, DDF>;
   constexpr int TPB = 64 / CPT;                              // threads per brick: 32 or 64 (a brick never shares a warp)
   const int lane = threadIdx.x & 31;
   const int sub = threadIdx.x % TPB;                         // thread index inside its brick
@@ -577,7 +581,7 @@ KernelSet make_kernel_set(const char* name, const char* bricks_name) {
   k.sweep = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, false>;
   k.sweep_bricks = nullptr;
   k.bricks_name = bricks_name;
-  k.brick_cells_per_cta = brick_cells_per_cta<Q, DDF>;
+  k.brick_cells_per_cta = brick_cells_per_cta<Q, T, DDF>;
   if constexpr (has_bricks<Q, T, COLL, DDF>) k.sweep_bricks = (const void*)&sweep_kernel<Q, T, COLL, DDF, SENSOR, true>;
   k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;
   k.couple = (const void*)&init_coupling_kernel<Q, T, COLL, DDF, SENSOR>;
