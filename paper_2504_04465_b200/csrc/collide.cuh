@@ -149,6 +149,8 @@ __device__ __forceinline__ void moments(const ModelParams& p, const T (&f)[Q], c
 }
 
 // ------------------------------------------------------------------ numerical equilibrium
+__host__ __device__ constexpr int ipow_c(int b, int e) { int r = 1; for (int k = 0; k < e; ++k) r *= b; return r; }
+
 // x^N for a compile-time N >= 0 by binary exponentiation (identical sub-powers are shared by the compiler)
 template <int N, typename T>
 __device__ __forceinline__ T ipow(T x) {
@@ -216,24 +218,43 @@ __device__ __forceinline__ void numeq_eval(T rho, const T (&m)[NLAMBDA], const T
   for (int a = 0; a < NLAMBDA; ++a) G[a] -= m[a];
 }
 
+// sum_i f_i x_i^PX y_i^PY (x_i^2 + y_i^2)^PR over the directions where the weight is not zero
+template <int Q, typename T, int PX, int PY, int PR>
+__device__ __forceinline__ T lattice_moment(const T (&f)[Q]) {
+  T s = T(0);
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I];
+    constexpr int wgt = ipow_c(x, PX) * ipow_c(y, PY) * ipow_c(x * x + y * y, PR);
+    if constexpr (wgt != 0) s += f[I] * T(wgt);
+  });
+  return s;
+}
+
 // Newton direction: solve (-J) d = G, -J = sum_i f_i M_i M_i^T (symmetric positive definite), by Cholesky.
+// The 36 entries of the lower triangle are 27 distinct lattice moments of f; the eight of the first column are the
+// moment sums the residual already holds (sum_i f_i M_ia = G_a + m_a), three more are sums of two others, so 16 sums
+// over the lattice are formed instead of 36 (the Jacobian was about half of the solve's arithmetic).
 // Returns false if the matrix is not positive definite.
 template <int Q, typename T>
-__device__ __forceinline__ bool newton_direction(const T (&f)[Q], const T (&G)[NLAMBDA], T (&d)[NLAMBDA]) {
+__device__ __forceinline__ bool newton_direction(const T (&f)[Q], const T (&G)[NLAMBDA], const T (&m)[NLAMBDA], T (&d)[NLAMBDA]) {
   T A[NLAMBDA][NLAMBDA];   // lower triangle used
-  static_for<0, NLAMBDA>([&](auto ac) {
-    constexpr int a = decltype(ac)::value;
-    static_for<0, a + 1>([&](auto bc) {
-      constexpr int b = decltype(bc)::value;
-      T s = T(0);
-      static_for<0, Q>([&](auto ic) {
-        constexpr int I = decltype(ic)::value;
-        constexpr int M = monomial(Lat<Q>::t, I, a) * monomial(Lat<Q>::t, I, b);
-        if constexpr (M != 0) s += f[I] * T(M);
-      });
-      A[a][b] = s;
-    });
-  });
+#pragma unroll
+  for (int a = 0; a < NLAMBDA; ++a) A[a][0] = G[a] + m[a];            // 1, x, y, xx, xy, yy, x r2, y r2
+  A[1][1] = A[3][0]; A[2][1] = A[4][0]; A[2][2] = A[5][0];
+  const T xxx = lattice_moment<Q, T, 3, 0, 0>(f), xxy = lattice_moment<Q, T, 2, 1, 0>(f);
+  const T xyy = lattice_moment<Q, T, 1, 2, 0>(f), yyy = lattice_moment<Q, T, 0, 3, 0>(f);
+  const T x4 = lattice_moment<Q, T, 4, 0, 0>(f), x3y = lattice_moment<Q, T, 3, 1, 0>(f), xxyy = lattice_moment<Q, T, 2, 2, 0>(f);
+  const T xy3 = lattice_moment<Q, T, 1, 3, 0>(f), y4 = lattice_moment<Q, T, 0, 4, 0>(f);
+  const T xxr2 = x4 + xxyy, xyr2 = x3y + xy3, yyr2 = xxyy + y4;
+  const T x3r2 = lattice_moment<Q, T, 3, 0, 1>(f), xxyr2 = lattice_moment<Q, T, 2, 1, 1>(f);
+  const T xyyr2 = lattice_moment<Q, T, 1, 2, 1>(f), y3r2 = lattice_moment<Q, T, 0, 3, 1>(f);
+  A[3][1] = xxx; A[4][1] = xxy; A[5][1] = xyy; A[6][1] = xxr2; A[7][1] = xyr2;
+  A[3][2] = xxy; A[4][2] = xyy; A[5][2] = yyy; A[6][2] = xyr2; A[7][2] = yyr2;
+  A[3][3] = x4; A[4][3] = x3y; A[5][3] = xxyy; A[6][3] = x3r2; A[7][3] = xxyr2;
+  A[4][4] = xxyy; A[5][4] = xy3; A[6][4] = xxyr2; A[7][4] = xyyr2;
+  A[5][5] = y4; A[6][5] = xyyr2; A[7][5] = y3r2;
+  A[6][6] = lattice_moment<Q, T, 2, 0, 2>(f); A[7][6] = lattice_moment<Q, T, 1, 1, 2>(f); A[7][7] = lattice_moment<Q, T, 0, 2, 2>(f);
   // A = C C^T, in place; the reciprocal of the diagonal is kept in rd
   T rd[NLAMBDA];
   bool ok = true;
@@ -314,7 +335,7 @@ __device__ __forceinline__ int feq_numerical(const ModelParams& p, T rho, T ux, 
     for (int a = 0; a < NLAMBDA; ++a) r1 += Num<T>::abs_(G[a]);
     converged = r1 <= tol;
     phase = (converged || it >= p.newton_max_iter) ? POLISH : SEARCH;    // then one unconditional full Newton step
-    if (!newton_direction<Q, T>(f, G, d)) { bad = true; break; }
+    if (!newton_direction<Q, T>(f, G, m, d)) { bad = true; break; }
     n0 = norm2sq(G);
     t = T(1);
   }
