@@ -231,7 +231,7 @@ __device__ __forceinline__ T lattice_moment(const T (&f)[Q]) {
   return s;
 }
 
-// Newton direction: solve (-J) d = G, -J = sum_i f_i M_i M_i^T (symmetric positive definite), by Cholesky.
+// Newton direction: solve (-J) d = G, -J = sum_i f_i M_i M_i^T (symmetric positive definite), by L D L^T.
 // The 36 entries of the lower triangle are 27 distinct lattice moments of f; the eight of the first column are the
 // moment sums the residual already holds (sum_i f_i M_ia = G_a + m_a), three more are sums of two others, so 16 sums
 // over the lattice are formed instead of 36 (the Jacobian was about half of the solve's arithmetic).
@@ -255,36 +255,42 @@ __device__ __forceinline__ bool newton_direction(const T (&f)[Q], const T (&G)[N
   A[4][4] = xxyy; A[5][4] = xy3; A[6][4] = xxyr2; A[7][4] = xyyr2;
   A[5][5] = y4; A[6][5] = xyyr2; A[7][5] = y3r2;
   A[6][6] = lattice_moment<Q, T, 2, 0, 2>(f); A[7][6] = lattice_moment<Q, T, 1, 1, 2>(f); A[7][7] = lattice_moment<Q, T, 0, 2, 2>(f);
-  // A = C C^T, in place; the reciprocal of the diagonal is kept in rd
-  T rd[NLAMBDA];
+  // A = L D L^T in place (unit lower L below the diagonal, D on it): the square-root-free form of the Cholesky
+  // factorisation -- the same direction up to rounding, but each column waits for one refined reciprocal (5 dependent
+  // instructions) instead of a square root and a division (~40), which matters with two warps per scheduler.
+  T rd[NLAMBDA];           // 1 / D_j
   bool ok = true;
   static_for<0, NLAMBDA>([&](auto jc) {
     constexpr int j = decltype(jc)::value;
+    T v[j > 0 ? j : 1];    // v_k = L_jk D_k
     T s = A[j][j];
-    static_for<0, j>([&](auto kc) { constexpr int k = decltype(kc)::value; s -= A[j][k] * A[j][k]; });
+    static_for<0, j>([&](auto kc) {
+      constexpr int k = decltype(kc)::value;
+      v[k] = A[j][k] * A[k][k];
+      s -= A[j][k] * v[k];
+    });
     if (!(s > T(0))) ok = false;
-    const T cjj = Num<T>::sqrt_(s);
-    A[j][j] = cjj;
-    rd[j] = T(1) / cjj;
+    A[j][j] = s;
+    rd[j] = fast_rcp(s);
     static_for<j + 1, NLAMBDA>([&](auto ic) {
       constexpr int i = decltype(ic)::value;
       T t = A[i][j];
-      static_for<0, j>([&](auto kc) { constexpr int k = decltype(kc)::value; t -= A[i][k] * A[j][k]; });
+      static_for<0, j>([&](auto kc) { constexpr int k = decltype(kc)::value; t -= A[i][k] * v[k]; });
       A[i][j] = t * rd[j];
     });
   });
-  T y[NLAMBDA];
-  static_for<0, NLAMBDA>([&](auto ic) {
+  T z[NLAMBDA];
+  static_for<0, NLAMBDA>([&](auto ic) {          // L z = G
     constexpr int i = decltype(ic)::value;
     T t = G[i];
-    static_for<0, i>([&](auto kc) { constexpr int k = decltype(kc)::value; t -= A[i][k] * y[k]; });
-    y[i] = t * rd[i];
+    static_for<0, i>([&](auto kc) { constexpr int k = decltype(kc)::value; t -= A[i][k] * z[k]; });
+    z[i] = t;
   });
-  static_for<0, NLAMBDA>([&](auto rc) {
+  static_for<0, NLAMBDA>([&](auto rc) {          // L^T d = D^-1 z
     constexpr int i = NLAMBDA - 1 - decltype(rc)::value;
-    T t = y[i];
+    T t = z[i] * rd[i];
     static_for<i + 1, NLAMBDA>([&](auto kc) { constexpr int k = decltype(kc)::value; t -= A[k][i] * d[k]; });
-    d[i] = t * rd[i];
+    d[i] = t;
   });
   return ok;
 }
