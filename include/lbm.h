@@ -149,6 +149,14 @@ int lbm_step(lbm_grid* g, int n_coarse_steps);
  * stopped inside the coarse step.  For tests and for timing sub-steps; lbm_step returns LBM_ESTATE unless the
  * fine-step count since the last coarse-step boundary is a multiple of 2^depth.  lbm_init_fields resets the count. */
 int lbm_step_fine(lbm_grid* g, int n_fine_steps);
+/* Time-dependent parameters of the paper's start-up ramps: the viscosity ramp (nu lowered linearly from 100 nu to nu
+ * over 20 convective times) is a sequence of lbm_set_relaxation calls (tau0 >= 1/2 of the finest level; tau_l follows Eq. 3),
+ * the Mach ramp (the state imposed by the Dirichlet / velocity-bounce-back sides raised to its nominal value over one
+ * convective time) a sequence of lbm_set_boundary_state calls (side 0..3; rho, u, T as in lbm_config).  Both take effect from
+ * the next lbm_step / lbm_step_fine call; they synchronise the stream and drop the captured graphs, which are re-captured on
+ * the next lbm_step (a few hundred microseconds: meant to be called once per coarse step, not per fine step). */
+int lbm_set_relaxation(lbm_grid* g, double tau0);
+int lbm_set_boundary_state(lbm_grid* g, int side, double rho, double ux, double uy, double T);
 /* Waits for the stream and returns the sticky device status: LBM_OK, LBM_EUNSTABLE or LBM_ENEWTON. */
 int lbm_sync(lbm_grid* g);
 

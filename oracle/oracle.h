@@ -73,6 +73,10 @@ int     orc_depth(const orc_grid* g);
 int64_t orc_num_cells(const orc_grid* g, int level);
 int64_t orc_num_ghosts(const orc_grid* g, int level);   /* coarse ghosts of interface (level, level-1) */
 double  orc_tau(const orc_grid* g, int level);
+/* start-up ramps (P:333 viscosity ramp, P:424 Mach ramp): new tau_0 (tau_l by Eq. 3) / new imposed state of one side,
+ * effective from the next update */
+int  orc_set_tau0(orc_grid* g, double tau0);
+int  orc_set_bc_state(orc_grid* g, int side, double rho, double ux, double uy, double T);
 /* storage-order tables of one level (caller-owned outputs, any may be NULL) */
 int  orc_get_cells(const orc_grid* g, int level, int32_t* ix, int32_t* iy, int32_t* type, int32_t* aux);
 int  orc_get_nbr(const orc_grid* g, int level, int32_t* nbr /* N*(Q-1), AoS, pull sources */);

@@ -59,6 +59,8 @@ def lib():
         L.orc_num_ghosts.restype = C.c_int64
         L.orc_tau.argtypes = [vp, C.c_int]
         L.orc_tau.restype = C.c_double
+        L.orc_set_tau0.argtypes = [vp, C.c_double]
+        L.orc_set_bc_state.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double]
         L.orc_newton_iterations.argtypes = [vp]
         L.orc_newton_iterations.restype = C.c_int64
         L.orc_cell_updates.argtypes = [vp]
@@ -168,6 +170,12 @@ class OracleGrid:
 
     def tau(self, l):
         return lib().orc_tau(self.h, l)
+
+    def set_tau0(self, tau0):
+        return lib().orc_set_tau0(self.h, float(tau0))
+
+    def set_bc_state(self, side, rho, ux, uy, T=0.0):
+        return lib().orc_set_bc_state(self.h, int(side), float(rho), float(ux), float(uy), float(T))
 
     def cells(self, l):
         n = self.n[l]

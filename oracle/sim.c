@@ -238,6 +238,22 @@ int orc_depth(const orc_grid* g) { return g->depth; }
 int64_t orc_num_cells(const orc_grid* g, int l) { return (l < 0 || l > g->depth) ? -1 : g->lv[l].n; }
 int64_t orc_num_ghosts(const orc_grid* g, int l) { return (l < 1 || l > g->depth) ? 0 : g->lv[l].ng; }
 double orc_tau(const orc_grid* g, int l) { return g->lv[l].tau; }
+
+/* Time-dependent parameters of the start-up ramps (viscosity ramp P:333: nu decreased linearly from 100 nu to nu; Mach
+ * ramp P:424: the state imposed by the Dirichlet sides raised to its nominal value): they act from the next update on.
+ * tau_l follows Eq. 3 (reading S3) from the new tau_0. */
+int orc_set_tau0(orc_grid* g, double tau0) {
+  if (!g || !(tau0 >= 0.5)) return ORC_EINVAL;
+  g->cfg.tau0 = tau0;
+  for (int l = 0; l <= g->depth; ++l) g->lv[l].tau = 0.5 + (tau0 - 0.5) / (double)((int64_t)1 << l);
+  return ORC_OK;
+}
+
+int orc_set_bc_state(orc_grid* g, int side, double rho, double ux, double uy, double T) {
+  if (!g || side < 0 || side > 3) return ORC_EINVAL;
+  g->cfg.bc_rho[side] = rho; g->cfg.bc_ux[side] = ux; g->cfg.bc_uy[side] = uy; g->cfg.bc_T[side] = T;
+  return ORC_OK;
+}
 int64_t orc_newton_iterations(const orc_grid* g) { return g->newton_its; }
 int64_t orc_cell_updates(const orc_grid* g) { return g->cell_updates; }
 

@@ -428,22 +428,13 @@ int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream
   g->bricks = g->ks->sweep_bricks != nullptr;
   if (const char* e = getenv("LBM_NO_BRICKS")) g->bricks = g->bricks && !(e[0] == '1');
   if (const char* e = getenv("LBM_BRICK_MIN_CELLS")) g->brick_min_cells = atoll(e);
-  // graphs: one coarse step from either parity of the coarsest level, and K steps for launch-bound grids
-  for (int p = 0; p < 2; ++p) {
-    int rc = capture(g, p, 1, &g->g1[p]);
-    if (rc) return rc;
-  }
+  // graphs (one coarse step from either parity of the coarsest level; K steps for launch-bound grids) are captured on
+  // first use by lbm_step and dropped when a parameter baked into their kernel arguments changes
   g->K = 0;
   if (g->launches_per_coarse > 0 && g->launches_per_coarse <= 32) {
     int K = (int)(128 / g->launches_per_coarse);
     K -= K & 1;
-    if (K >= 2) {
-      g->K = K;
-      for (int p = 0; p < 2; ++p) {
-        int rc = capture(g, p, K, &g->gk[p]);
-        if (rc) return rc;
-      }
-    }
+    if (K >= 2) g->K = K;
   }
   return LBM_OK;
 }
@@ -516,6 +507,12 @@ int lbm_step(lbm_grid* g, int n) {
   if (!g->bound || !g->inited) return LBM_ESTATE;
   if (g->kfine != 0) return LBM_ESTATE;           // graphs start at a coarse-step boundary
   int& p = g->dl[g->depth].cur;
+  // capture what this call needs before the timed region starts: n = nk launches of the K-step graph (parity kept) and
+  // r single steps that alternate the parity
+  const int nk = g->K >= 2 ? n / g->K : 0, r = n - nk * g->K;
+  if (nk > 0 && !g->gk[p]) { int rc = capture(g, p, g->K, &g->gk[p]); if (rc) return rc; }
+  if (r >= 1 && !g->g1[p]) { int rc = capture(g, p, 1, &g->g1[p]); if (rc) return rc; }
+  if (r >= 2 && !g->g1[p ^ 1]) { int rc = capture(g, p ^ 1, 1, &g->g1[p ^ 1]); if (rc) return rc; }
   CK(cudaEventRecord(g->ev0, g->stream));
   while (n > 0) {
     if (g->K >= 2 && n >= g->K) {
@@ -529,6 +526,33 @@ int lbm_step(lbm_grid* g, int n) {
   }
   CK(cudaEventRecord(g->ev1, g->stream));
   g->timed = true;
+  return LBM_OK;
+}
+
+namespace {
+void drop_graphs(lbm_grid* g) {
+  if (!g->bound) return;
+  cudaStreamSynchronize(g->stream);
+  for (int p = 0; p < 2; ++p) {
+    if (g->g1[p]) { cudaGraphExecDestroy(g->g1[p]); g->g1[p] = nullptr; }
+    if (g->gk[p]) { cudaGraphExecDestroy(g->gk[p]); g->gk[p] = nullptr; }
+  }
+}
+}  // namespace
+
+int lbm_set_relaxation(lbm_grid* g, double tau0) {
+  if (!g || !(tau0 >= 0.5)) return LBM_EINVAL;
+  g->hg.cfg.tau0 = tau0;
+  for (int l = 0; l <= g->depth; ++l) g->hg.lv[l].tau = 0.5 + (tau0 - 0.5) / (double)((int64_t)1 << l);   // Eq. 3 (S3)
+  drop_graphs(g);
+  return LBM_OK;
+}
+
+int lbm_set_boundary_state(lbm_grid* g, int side, double rho, double ux, double uy, double T) {
+  if (!g || side < 0 || side > 3) return LBM_EINVAL;
+  g->hg.cfg.bc_rho[side] = rho; g->hg.cfg.bc_ux[side] = ux; g->hg.cfg.bc_uy[side] = uy; g->hg.cfg.bc_T[side] = T;
+  g->mp.bc_rho[side] = rho; g->mp.bc_ux[side] = ux; g->mp.bc_uy[side] = uy; g->mp.bc_T[side] = T;
+  drop_graphs(g);
   return LBM_OK;
 }
 

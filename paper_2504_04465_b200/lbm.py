@@ -23,7 +23,7 @@ _ERR = {EINVAL: "LBM_EINVAL", ENOMEM: "LBM_ENOMEM", EMESH: "LBM_EMESH", ECUDA: "
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
-           "lbm_get_schedule", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_sync", "lbm_get_macroscopic",
+           "lbm_get_schedule", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic",
            "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_measure_fma_peak"]
 
 
@@ -79,6 +79,8 @@ def lib():
         L.lbm_init_fields.argtypes = [vp, vp, vp, vp, vp]
         L.lbm_step.argtypes = [vp, C.c_int]
         L.lbm_step_fine.argtypes = [vp, C.c_int]
+        L.lbm_set_relaxation.argtypes = [vp, C.c_double]
+        L.lbm_set_boundary_state.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double]
         L.lbm_sync.argtypes = [vp]
         L.lbm_get_macroscopic.argtypes = [vp, vp, vp, vp, vp]
         L.lbm_get_populations.argtypes = [vp, C.c_int, C.c_int, vp]
@@ -234,6 +236,12 @@ class Grid:
 
     def step_fine(self, n=1):
         _check("lbm_step_fine", lib().lbm_step_fine(self.h, int(n)))
+
+    def set_tau0(self, tau0):
+        _check("lbm_set_relaxation", lib().lbm_set_relaxation(self.h, float(tau0)))
+
+    def set_bc_state(self, side, rho, ux, uy, T=0.0):
+        _check("lbm_set_boundary_state", lib().lbm_set_boundary_state(self.h, int(side), float(rho), float(ux), float(uy), float(T)))
 
     def sync(self):
         return lib().lbm_sync(self.h)

@@ -337,6 +337,20 @@ def stripe(nc=32, lo=8, hi=24, lattice=9, collision=BGK, tau0=0.8, fields=None, 
     return Case("stripe", mesh, lattice=lattice, collision=collision, tau0=tau0, bc=(BC_PERIODIC,) * 4, fields=fields, **kw)
 
 
+# ----------------------------------------------------------------------------- start-up ramps
+def viscosity_ramp_tau0(tau0, step, nsteps, factor=100.0):
+    """tau_0 at coarse step `step` of the viscosity ramp: nu starts at factor * nu and decreases linearly to nu over
+    nsteps steps; tau - 1/2 is proportional to nu on every level (Eq. 3), so the ramp scales tau_0 - 1/2."""
+    m = factor - (factor - 1.0) * min(step / float(nsteps), 1.0)
+    return 0.5 + (tau0 - 0.5) * m
+
+
+def mach_ramp_factor(step, nsteps, start=0.5):
+    """Fraction of the nominal boundary velocity imposed at coarse step `step` of the Mach ramp (the free-stream Mach
+    number starts below the target and is raised to it over one convective time)."""
+    return start + (1.0 - start) * min(step / float(nsteps), 1.0)
+
+
 def eval_fields(case, levels_ix_iy):
     """levels_ix_iy: list over levels 0..depth of (ix, iy) arrays in storage order -> flat rho, ux, uy, T."""
     out = [[], [], [], []]

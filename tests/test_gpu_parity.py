@@ -229,3 +229,42 @@ def test_sod_numerical_equilibrium_fp64_and_fp32(lattice, mesh):
         d = max_pop_diff(g, o, (0, 1))
         assert d <= tol * 8.0, (lattice, mesh, prec, d)      # populations scale with rho <= 8 (Eq. 12)
         g.close()
+
+
+# ------------------------------------------------------------------ start-up ramps
+def test_viscosity_and_lid_velocity_ramp_cavity():
+    """lbm_set_relaxation / lbm_set_boundary_state once per coarse step (graphs re-captured) against the oracle's setters:
+    two-level cavity, nu from 100 nu down to nu and the lid velocity from half to full over 8 coarse steps, then 4 more."""
+    case = W.cavity(scale=0.25)
+    g = gpu_from_case(case, 64)
+    o = oracle_from_case(case)
+    for step in range(12):
+        tau0 = W.viscosity_ramp_tau0(case.tau0, step, 8)
+        ulid = case.bc_ux[3] * W.mach_ramp_factor(step, 8)
+        g.set_tau0(tau0)
+        g.set_bc_state(3, 1.0, ulid, 0.0)
+        assert o.set_tau0(tau0) == 0 and o.set_bc_state(3, 1.0, ulid, 0.0) == 0
+        g.step(1)
+        assert o.step(1) == 0
+    assert g.sync() == 0
+    assert o.tau(0) == pytest.approx(case.tau0) and o.tau(1) == pytest.approx(0.5 + (case.tau0 - 0.5) / 2)
+    assert max_pop_diff(g, o) <= 1e-12
+    g.close()
+
+
+def test_mach_ramp_on_dirichlet_sides_naca():
+    """Numerical-equilibrium Dirichlet sides driven through the Mach ramp of P:424."""
+    case = W.naca(chord=64, depth=3, radii=(1, 2.5, 5))
+    g = gpu_from_case(case, 64)
+    o = oracle_from_case(case)
+    for step in range(4):
+        m = W.mach_ramp_factor(step, 3, start=0.8)
+        for side in (0, 2, 3):
+            args = (side, case.bc_rho[side], case.bc_ux[side] * m, case.bc_uy[side] * m, case.bc_T[side])
+            g.set_bc_state(*args)
+            assert o.set_bc_state(*args) == 0
+        g.step(1)
+        assert o.step(1) == 0
+    assert g.sync() == 0
+    assert max_pop_diff(g, o, (0, 1)) <= 1e-12
+    g.close()

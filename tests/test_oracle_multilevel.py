@@ -304,3 +304,17 @@ def test_multilevel_vs_uniform_fine_converges():
         errs.append(e)
     assert errs[0] < 0.05
     assert errs[1] < errs[0] / 1.6
+
+
+def test_ramp_setters_follow_eq3_and_reject_bad_arguments():
+    """orc_set_tau0: tau_l - 1/2 = (tau_0 - 1/2) / 2^l (Eq. 3, S3) on every level; tau_0 < 1/2 and a side outside 0..3 are
+    rejected; the viscosity-ramp helper starts at 100 nu and ends at nu."""
+    case = W.patch(nc=48, lo=8, hi=40, depth=2)
+    o = oracle_from_case(case, init=False)
+    assert o.set_tau0(0.9) == 0
+    for l in range(3):
+        assert o.tau(l) == pytest.approx(0.5 + 0.4 / 2 ** l, abs=1e-15)
+    assert o.set_tau0(0.49) != 0 and o.set_bc_state(4, 1.0, 0.0, 0.0) != 0
+    assert W.viscosity_ramp_tau0(0.6, 0, 10) == pytest.approx(0.5 + 0.1 * 100)
+    assert W.viscosity_ramp_tau0(0.6, 10, 10) == pytest.approx(0.6) and W.viscosity_ramp_tau0(0.6, 25, 10) == pytest.approx(0.6)
+    assert W.mach_ramp_factor(0, 4) == 0.5 and W.mach_ramp_factor(4, 4) == 1.0
