@@ -87,7 +87,7 @@ def algorithmic_bytes_per_update(case, precision):
 def moved_bytes_per_update(g, case, precision):
     """Bytes this implementation has to move per cell update, weighted over the levels by their share of the updates:
     a cell of a regular brick needs its 2*npop reals and 36 B of tile bases per 64 cells; any
-    other cell the list row, the type byte and its entry of the irregular-cell list on top."""
+    other cell the list row and the type byte on top, plus its entry of the irregular-cell list on levels that have bricks."""
     Q = case.lattice
     npop = Q * (2 if case.ddf else 1) + (8 if case.collision == W.NUMEQ else 0)
     s = precision // 8
@@ -96,7 +96,7 @@ def moved_bytes_per_update(g, case, precision):
     for l in range(g.depth + 1):
         nb = 64 * int(g.info.n_bricks[l]) if bricks and g.n[l] >= int(g.info.brick_min_level_cells) else 0
         k = 1 << (g.depth - l)
-        tot += k * (nb * (2 * npop * s + 36.0 / 64) + (g.n[l] - nb) * (2 * npop * s + (Q - 1) * 4 + 1 + (4 if bricks else 0)))
+        tot += k * (nb * (2 * npop * s + 36.0 / 64) + (g.n[l] - nb) * (2 * npop * s + (Q - 1) * 4 + 1 + (4 if nb else 0)))
         upd += k * g.n[l]
     return tot / upd
 

@@ -51,3 +51,29 @@ def test_reference_arm_under_torchrun_prints_one_line():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["cpu_baseline"]["kind"] == "oracle" and d["value"] > 0
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["unit"] == "MLUPS"
+
+
+def test_algorithmic_bytes_per_update_match_the_scope_table():
+    """SURVEY 8(d) / DESIGN.md Sec. 11: 2*npop*s + (Q-1)*4 + 4 bytes per cell update of the list-addressed method."""
+    import bench
+    from paper_2504_04465_b200 import workloads as W
+    assert bench.algorithmic_bytes_per_update(W.tgv(64), 64) == 180
+    assert bench.algorithmic_bytes_per_update(W.tgv(64), 32) == 108
+    assert bench.algorithmic_bytes_per_update(W.tgv(64, lattice=13, collision=W.RR), 64) == 260
+    assert bench.algorithmic_bytes_per_update(W.tgv(64, lattice=21, collision=W.RR), 64) == 420
+    assert bench.algorithmic_bytes_per_update(W.riemann(n=64), 64) == 1332
+    assert bench.algorithmic_bytes_per_update(W.naca(chord=64, depth=3, radii=(1, 2.5, 5)), 64) == 884
+    # Table 3a of the paper is carried verbatim (P:656-663)
+    assert bench.PAPER_TABLE3[(21, "unif")] == 618.5 and bench.PAPER_TABLE3[(37, "band")] == 307.4 and len(bench.PAPER_TABLE3) == 12
+
+
+def test_moved_bytes_count_bricks_only_on_large_levels():
+    """Bytes the implementation must move: a 64^2 box is below the 2^18-cell threshold (list: 2*9*8 + 32 + 1 B),
+    a 1024^2 box is all bricks (144 B + 36 B per 64 cells)."""
+    import bench
+    from paper_2504_04465_b200 import lbm, workloads as W
+    small = lbm.Grid.from_case(W.tgv(64))
+    assert bench.moved_bytes_per_update(small, W.tgv(64), 64) == 2 * 9 * 8 + 32 + 1
+    big = lbm.Grid.from_case(W.tgv(1024))
+    assert bench.moved_bytes_per_update(big, W.tgv(1024), 64) == pytest.approx(144 + 36 / 64)
+    small.close(); big.close()
