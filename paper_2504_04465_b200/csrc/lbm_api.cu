@@ -151,15 +151,17 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   a.nbrick = (int)L.nbrick; a.n_irr = (int)L.n_irr;
   const int64_t cells_per_cta = g->ks->brick_cells_per_cta;
   a.brick_ctas = (int)((L.nbrick * 64 + cells_per_cta - 1) / cells_per_cta);
+  a.list_ctas = (int)((L.n_irr + BLOCK - 1) / BLOCK);
   // Small levels are latency-bound, not traffic-bound: they go through the list with ONE cell per thread (the list part
   // of the brick kernel with no bricks and no indirection), which gives them the most threads; measured on the 39 k-cell
   // cavity: fp64 7.4 against 6.6 GLUPS with bricks (two cells per thread).
   int rc;
   if (g->bricks && L.n < g->brick_min_cells) {
     a.nbrick = 0; a.brick_ctas = 0; a.irr = nullptr; a.n_irr = (int)L.n;
-    rc = launch_grid(g->ks->sweep_bricks, (unsigned)((L.n + BLOCK - 1) / BLOCK), &a, &g->mp, g->stream, g->pdl);
+    a.list_ctas = (int)((L.n + BLOCK - 1) / BLOCK);
+    rc = launch_grid(g->ks->sweep_bricks, (unsigned)a.list_ctas, &a, &g->mp, g->stream, g->pdl);
   } else if (g->bricks && L.nbrick > 0) {
-    rc = launch_grid(g->ks->sweep_bricks, (unsigned)(a.brick_ctas + (L.n_irr + BLOCK - 1) / BLOCK), &a, &g->mp, g->stream, g->pdl);
+    rc = launch_grid(g->ks->sweep_bricks, (unsigned)(a.list_ctas + a.brick_ctas), &a, &g->mp, g->stream, g->pdl);
   } else {
     rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream, g->ks->cells_per_thread, g->pdl);
   }

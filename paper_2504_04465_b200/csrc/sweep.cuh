@@ -38,12 +38,13 @@ struct LevelArgs {
   long long fps;            // its plane stride
   double tau;
   int* status;              // sticky FLAG_* word
-  // compressed addressing (BRICKS kernels): the first brick_ctas CTAs update regular bricks through tile arithmetic,
-  // the others the n_irr remaining cells irr[] through the list
+  // compressed addressing (BRICKS kernels): the first list_ctas CTAs update the n_irr irregular cells irr[] through the
+  // list (first, so that the slower one-cell-per-thread work is not the tail of the launch), the following brick_ctas
+  // CTAs the regular bricks through tile arithmetic
   const int* brick_nb;      // [nbrick][9] first storage index of the 3x3 tiles around (and of, k = 4) the brick
   const unsigned short* brick_tab;   // [(Q-1)][64] (k << 6) | Z-position of the pull source
   const int* irr;
-  int nbrick, n_irr, brick_ctas;
+  int nbrick, n_irr, brick_ctas, list_ctas;
 };
 
 template <int Q, bool DDF, int COLL>
@@ -91,14 +92,14 @@ template <int Q, typename T, bool DDF> constexpr int BRICK_CPT = (Q * (DDF ? 2 :
 template <int Q, typename T, bool DDF> constexpr int brick_cells_per_cta = 128 * BRICK_CPT<Q, T, DDF>;
 
 template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
-__device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelParams& p) {
+__device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelParams& p, int block) {
   using PL = PopLayout<Q, DDF, COLL>;
   constexpr int CPT = BRICK_CPT<Q, T, DDF>;
   constexpr int TPB = 64 / CPT;                              // threads per brick: 32 or 64 (a brick never shares a warp)
   const int lane = threadIdx.x & 31;
   const int sub = threadIdx.x % TPB;                         // thread index inside its brick
   constexpr int grp = 0;                                     // lanes 0-8 of every warp hold the tile bases
-  const int brick_raw = (blockIdx.x * 128 + threadIdx.x) / TPB;
+  const int brick_raw = (block * 128 + threadIdx.x) / TPB;
   if (brick_raw >= a.nbrick) return;                         // whole warp beyond the last brick
   const int brick = brick_raw;
   const int m0 = sub * CPT;                                  // Z-position of this thread's first cell
@@ -173,11 +174,11 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
   int c0;
   if constexpr (BRICKS) {
     static_assert(has_bricks<Q, T, COLL, DDF>, "no brick path for this model");
-    if ((int)blockIdx.x < a.brick_ctas) {
-      brick_update<Q, T, COLL, DDF, SENSOR>(a, p);
+    if ((int)blockIdx.x >= a.list_ctas) {
+      brick_update<Q, T, COLL, DDF, SENSOR>(a, p, (int)blockIdx.x - a.list_ctas);
       return;
     }
-    const int t = ((int)blockIdx.x - a.brick_ctas) * blockDim.x + threadIdx.x;
+    const int t = (int)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= a.n_irr) return;
     c0 = a.irr ? a.irr[t] : t;              // irr == null: every cell of a small level through the list, one per thread
   } else {
