@@ -231,6 +231,31 @@ def aggregate_mlups(updates_per_rank_step, steps, world, ms):
     return updates_per_rank_step * steps * world / (ms * 1e-3) / 1e6
 
 
+def also_measure(lbm, name, precision, dev, peak):
+    """Device-resident throughput of another workload with its default step count, for the `also` entries of the default
+    line (same timing rules: 3 warm-up steps, CUDA events on the bound stream around the replayed graphs)."""
+    case, info = make_case(name, 1.0)
+    g = lbm.Grid.from_case(case, precision=precision)
+    g.bind(dev)
+    cells = [g.cells(l)[:2] for l in range(g.depth + 1)]
+    rc = g.init_fields(*W.eval_fields(case, cells))
+    assert rc == 0, rc
+    g.step(3)
+    assert g.sync() == 0
+    g.step(info["steps"])
+    ms = g.last_step_ms()
+    assert g.sync() == 0
+    upd = int(g.info.updates_per_coarse_step)
+    bpu = algorithmic_bytes_per_update(case, precision)
+    v = upd * info["steps"] / (ms * 1e-3) / 1e6
+    out = {"workload": info["workload"], "dtype": "f%d" % precision, "value": v, "unit": "MLUPS", "steps": info["steps"],
+           "ms_per_step": ms / info["steps"], "cells": g.ntot, "gpu_launches": int(g.info.launches_per_coarse_step) * info["steps"],
+           "roofline_frac": v * 1e6 * bpu / 1e9 / peak, "roofline_frac_moved": v * 1e6 * moved_bytes_per_update(g, case, precision) / 1e9 / peak,
+           "kernel": g.kernel_name()}
+    g.close()
+    return out
+
+
 # ----------------------------------------------------------------------------- CUDA arm
 def main():
     ap = argparse.ArgumentParser()
@@ -243,6 +268,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0, help="0 disables the cpu_baseline leg")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--also", default=None, help="comma list of other workloads measured briefly into the line's `also` "
+                    "(default for the default workload: cavity = configs[1] and uniform = configs[0] scaled; 'none' disables)")
     args = ap.parse_args()
     case, info = make_case(args.workload, args.scale)
     if args.steps is None:
@@ -401,6 +428,10 @@ def main():
     elif "fp64_pipe_pct" in counters:
         line["roofline"]["fp64_pipe_pct_ncu"] = counters["fp64_pipe_pct"]
         line["roofline"]["fp64_tflops"] = upd * K * counters["fp64_flop_per_update"] / (ms * 1e-3) / 1e12
+    also = args.also if args.also is not None else ("cavity,uniform" if args.workload == "cylinder" and args.scale == 1.0 else "none")
+    if also != "none" and world == 1:
+        g.close()                # release the arena before building the next grid
+        line["also"] = [also_measure(lbm, w, args.precision, dev, peak) for w in also.split(",") if w]
     if args.cpu_baseline_seconds > 0 and world >= 1:
         o = oracle_grid(case)
         v, nf, nu, dt = oracle_rate(o, args.cpu_baseline_seconds)
