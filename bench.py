@@ -46,6 +46,10 @@ def make_case(name, scale):
     if name == "cylinder":
         D = int(round(200 * scale))
         return W.cylinder(D=D), dict(workload="cylinder (BASELINE configs[2]): D2Q9-RR, D=%d, 64Dx64D, 6 levels" % D, steps=300)
+    if name == "cylinder:sponge":     # configs[2] with the paper's far-field pressure relaxation (Eq. 10-11) switched on
+        D = int(round(200 * scale))
+        return W.cylinder(D=D, sponge_d=(24, 30, 0.1)), dict(
+            workload="cylinder + sponge (Eq. 10-11: sigma 0 -> 0.1 between 24 D and 30 D): D2Q9-RR, D=%d, 6 levels" % D, steps=300)
     if name == "uniform":
         n = int(round(4096 * scale))
         return W.tgv(n), dict(workload="uniform periodic %dx%d tree-stored D2Q9-BGK Taylor-Green (configs[0] scaled)" % (n, n), steps=4000)

@@ -73,6 +73,11 @@ typedef struct {
   double sensor_A;    /* Eq. 53 */
   double newton_tol;
   double bc_rho[4], bc_ux[4], bc_uy[4], bc_T[4];   /* imposed states per side (walls: velocity only) */
+  /* Pressure-relaxation sponge against acoustic reflections, Eq. 10-11 P:296-303 (reading S24 of DESIGN.md):
+   * sigma(r) = 0 for r < r0, rises linearly to sigma_max at r1 and stays there, r = distance of the cell centre from
+   * (x0, y0) in finest-level units; before each collision rho is relaxed to rho (1 - sigma) + sigma rho_inf at unchanged
+   * velocity and non-equilibrium part.  sigma_max = 0: off.  Weakly compressible models only (LBM_EINVAL otherwise). */
+  double sponge_x0, sponge_y0, sponge_r0, sponge_r1, sponge_sigma_max, sponge_rho_inf;
 } lbm_config;
 
 typedef struct {
@@ -121,6 +126,8 @@ int lbm_get_cells(const lbm_grid* g, int level, int32_t* ix, int32_t* iy, int32_
 int lbm_get_nbr(const lbm_grid* g, int level, int32_t* nbr);
 int lbm_get_ghosts(const lbm_grid* g, int level, int32_t* coarse, int32_t* child, uint64_t* mask);
 int lbm_get_schedule(const lbm_grid* g, int32_t* k_of, int32_t* level_of, int cap);
+/* sponge coefficient sigma of every stored cell of one level (Eq. 11; HOST out, n_cells[level] doubles; zeros when off) */
+int lbm_get_sponge(const lbm_grid* g, int level, double* sigma);
 /* Compressed addressing of the device path: a "brick" is an aligned 8x8 tile of level-`level`
  * cells that are all stored FLUID cells (hence 64 consecutive storage indices) and whose
  * every neighbour-list entry equals  tiles9[9*b + k] + z  with (k, z) = (table[(i-1)*64 + m] >> 6, & 63) for the

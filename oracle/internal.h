@@ -27,6 +27,7 @@ typedef struct {
   int32_t* g_child;     /* 4 per ghost: storage index on level-1 of child a+2b, -1 if absent */
   uint64_t* g_mask;     /* bit i set: direction i unknown (coalesced) */
   double tau;
+  double* sigma;        /* sponge coefficient per stored cell (Eq. 11), NULL when the sponge is off */
   double* S[2];         /* populations, AoS [cell][npop]: f(Q) | g(Q) | lambda(8) */
   int cur;              /* which of S[] is current */
 } orc_level;

@@ -56,6 +56,10 @@ typedef struct {
   double sensor_A;  /* Eq. 53 */
   double newton_tol;/* P:934 */
   double bc_rho[4], bc_ux[4], bc_uy[4], bc_T[4];
+  /* pressure-relaxation sponge, Eq. 10-11 P:296-303 (reading S24 of DESIGN.md): sigma(r) = 0 for r < r0, rises linearly to
+   * sigma_max at r1 and stays there, r = distance of the cell centre from (x0, y0) in finest-level units; before each
+   * collision rho is relaxed to rho(1-sigma) + sigma rho_inf.  sigma_max = 0: off.  Weakly compressible models only. */
+  double sponge_x0, sponge_y0, sponge_r0, sponge_r1, sponge_sigma_max, sponge_rho_inf;
 } orc_config;
 
 typedef struct orc_grid orc_grid;
@@ -75,6 +79,7 @@ int64_t orc_num_ghosts(const orc_grid* g, int level);   /* coarse ghosts of inte
 double  orc_tau(const orc_grid* g, int level);
 /* start-up ramps (P:333 viscosity ramp, P:424 Mach ramp): new tau_0 (tau_l by Eq. 3) / new imposed state of one side,
  * effective from the next update */
+int  orc_get_sponge(const orc_grid* g, int level, double* sigma /* one per stored cell */);
 int  orc_set_tau0(orc_grid* g, double tau0);
 int  orc_set_bc_state(orc_grid* g, int side, double rho, double ux, double uy, double T);
 /* storage-order tables of one level (caller-owned outputs, any may be NULL) */

@@ -38,6 +38,8 @@ class OrcConfig(C.Structure):
         ("tau0", C.c_double), ("T0", C.c_double), ("gamma", C.c_double), ("sensor_A", C.c_double),
         ("newton_tol", C.c_double),
         ("bc_rho", C.c_double * 4), ("bc_ux", C.c_double * 4), ("bc_uy", C.c_double * 4), ("bc_T", C.c_double * 4),
+        ("sponge_x0", C.c_double), ("sponge_y0", C.c_double), ("sponge_r0", C.c_double), ("sponge_r1", C.c_double),
+        ("sponge_sigma_max", C.c_double), ("sponge_rho_inf", C.c_double),
     ]
 
 
@@ -60,6 +62,7 @@ def lib():
         L.orc_tau.argtypes = [vp, C.c_int]
         L.orc_tau.restype = C.c_double
         L.orc_set_tau0.argtypes = [vp, C.c_double]
+        L.orc_get_sponge.argtypes = [vp, C.c_int, vp]
         L.orc_set_bc_state.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double]
         L.orc_newton_iterations.argtypes = [vp]
         L.orc_newton_iterations.restype = C.c_int64
@@ -89,8 +92,12 @@ def _ptr(a):
 
 def make_config(lattice=9, collision=BGK, ddf=0, sensor=0, trace_eq=0, depth=0, nx_coarse=1, ny_coarse=1,
                 tau0=0.6, T0=0.0, gamma=1.4, sensor_A=1.5, newton_tol=1e-12, newton_max_iter=50,
-                bc=(0, 0, 0, 0), bc_rho=(1, 1, 1, 1), bc_ux=(0, 0, 0, 0), bc_uy=(0, 0, 0, 0), bc_T=(0, 0, 0, 0)):
+                bc=(0, 0, 0, 0), bc_rho=(1, 1, 1, 1), bc_ux=(0, 0, 0, 0), bc_uy=(0, 0, 0, 0), bc_T=(0, 0, 0, 0),
+                sponge=None):
+    """sponge: None or (x0, y0, r0, r1, sigma_max, rho_inf) of Eq. 10-11."""
     c = OrcConfig()
+    if sponge is not None:
+        (c.sponge_x0, c.sponge_y0, c.sponge_r0, c.sponge_r1, c.sponge_sigma_max, c.sponge_rho_inf) = [float(v) for v in sponge]
     c.lattice, c.collision, c.ddf, c.sensor, c.trace_eq = lattice, collision, ddf, sensor, trace_eq
     c.depth, c.nx_coarse, c.ny_coarse, c.newton_max_iter = depth, nx_coarse, ny_coarse, newton_max_iter
     c.tau0, c.T0, c.gamma, c.sensor_A, c.newton_tol = tau0, T0, gamma, sensor_A, newton_tol
@@ -170,6 +177,11 @@ class OracleGrid:
 
     def tau(self, l):
         return lib().orc_tau(self.h, l)
+
+    def sponge(self, l):
+        a = np.zeros(self.n[l])
+        assert lib().orc_get_sponge(self.h, l, _ptr(a)) == 0
+        return a
 
     def set_tau0(self, tau0):
         return lib().orc_set_tau0(self.h, float(tau0))

@@ -134,6 +134,17 @@ static void update_level(orc_grid* g, int l)
       for (int a = 0; a < ORC_NLAMBDA; ++a)
         lam[a] = (type == ORC_COARSE_GHOST) ? coalesce(g, l, L->aux[c], off + a) /* Eq. 6 */ : own[off + a];
     }
+    /* pressure relaxation (Eq. 10, "applied before the collision step"; reading S24): rho -> rho' = rho (1 - sigma) +
+       sigma rho_inf at unchanged velocity and unchanged non-equilibrium part, i.e. f_i += (rho'/rho - 1) f_i^eq(rho, u)
+       (the polynomial equilibrium is linear in rho); a Neumann cell follows its source cell (S13) */
+    if (L->sigma && L->sigma[self] > 0.0) {
+      const double sg = L->sigma[self];
+      double rho = 0.0, jx = 0.0, jy = 0.0, dummy[ORC_NLAMBDA] = {0};
+      for (int i = 0; i < Q; ++i) { rho += f[i]; jx += orc_phys_cx(g->phys, i) * f[i]; jy += orc_phys_cy(g->phys, i) * f[i]; }
+      orc_phys_equilibrium(g->phys, rho, jx / rho, jy / rho, orc_phys_T0(g->phys), dummy, fo, go);
+      const double rho_new = rho * (1.0 - sg) + sg * g->cfg.sponge_rho_inf;
+      for (int i = 0; i < Q; ++i) f[i] += (rho_new / rho - 1.0) * fo[i];
+    }
     /* steps 2-5: moments, equilibrium, sensor, relaxation */
     int it = orc_phys_collide(g->phys, L->tau, f, gg, lam, fo, go);
     for (int i = 0; i < Q; ++i) out[i] = fo[i];
@@ -203,6 +214,10 @@ int orc_grid_create(const orc_config* cfg, const int64_t* split_off, const int32
   for (int s = 0; s < 4; ++s)
     if ((cfg->bc[s] == ORC_BC_MOVING_WALL || cfg->bc[s] == ORC_BC_INFLOW_VBB) && (cfg->ddf || cfg->collision == ORC_NUMEQ)) rc = ORC_EINVAL;
   if (!(cfg->tau0 >= 0.5)) rc = ORC_EINVAL;
+  /* the sponge relaxes rho = p / T0: weakly compressible models only */
+  if (cfg->sponge_sigma_max != 0.0 && (cfg->ddf || cfg->collision == ORC_NUMEQ || !(cfg->sponge_sigma_max > 0.0) ||
+                                       !(cfg->sponge_sigma_max <= 1.0) || !(cfg->sponge_r1 > cfg->sponge_r0) || !(cfg->sponge_r0 >= 0.0)))
+    rc = ORC_EINVAL;
   g->lv = (orc_level*)calloc((size_t)cfg->depth + 1, sizeof(orc_level));
   if (!g->lv) rc = ORC_ENOMEM;
   if (!rc) rc = orc_build_levels(g, split_off, split_xy, solid_off, solid_xy);
@@ -213,6 +228,20 @@ int orc_grid_create(const orc_config* cfg, const int64_t* split_off, const int32
     for (int b = 0; b < 2; ++b) {
       L->S[b] = (double*)calloc((size_t)(L->n * g->npop + 1), sizeof(double));
       if (!L->S[b]) rc = ORC_ENOMEM;
+    }
+    if (cfg->sponge_sigma_max > 0.0 && !rc) {
+      /* Eq. 11: linear ramp of sigma between r0 and r1 around (x0, y0), cell centres ((ix+1/2)h, (iy+1/2)h), h = 2^l */
+      L->sigma = (double*)calloc((size_t)L->n + 1, sizeof(double));
+      if (!L->sigma) { rc = ORC_ENOMEM; break; }
+      const double h = (double)((int64_t)1 << l);
+      for (int64_t c = 0; c < L->n; ++c) {
+        const double dx = (L->ix[c] + 0.5) * h - cfg->sponge_x0, dy = (L->iy[c] + 0.5) * h - cfg->sponge_y0;
+        const double r = sqrt(dx * dx + dy * dy);
+        double sg = 0.0;
+        if (r >= cfg->sponge_r1) sg = cfg->sponge_sigma_max;
+        else if (r >= cfg->sponge_r0) sg = cfg->sponge_sigma_max * (r - cfg->sponge_r0) / (cfg->sponge_r1 - cfg->sponge_r0);
+        L->sigma[c] = sg;
+      }
     }
   }
   if (rc) { orc_grid_destroy(g); return rc; }
@@ -227,7 +256,7 @@ void orc_grid_destroy(orc_grid* g)
     for (int l = 0; l <= g->depth; ++l) {
       orc_level* L = &g->lv[l];
       free(L->ix); free(L->iy); free(L->type); free(L->aux); free(L->nbr);
-      free(L->g_coarse); free(L->g_child); free(L->g_mask); free(L->S[0]); free(L->S[1]);
+      free(L->g_coarse); free(L->g_child); free(L->g_mask); free(L->S[0]); free(L->S[1]); free(L->sigma);
     }
   free(g->lv);
   free(g->phys);
@@ -242,6 +271,12 @@ double orc_tau(const orc_grid* g, int l) { return g->lv[l].tau; }
 /* Time-dependent parameters of the start-up ramps (viscosity ramp P:333: nu decreased linearly from 100 nu to nu; Mach
  * ramp P:424: the state imposed by the Dirichlet sides raised to its nominal value): they act from the next update on.
  * tau_l follows Eq. 3 (reading S3) from the new tau_0. */
+int orc_get_sponge(const orc_grid* g, int l, double* sigma) {
+  if (!g || !sigma || l < 0 || l > g->depth) return ORC_EINVAL;
+  for (int64_t c = 0; c < g->lv[l].n; ++c) sigma[c] = g->lv[l].sigma ? g->lv[l].sigma[c] : 0.0;
+  return ORC_OK;
+}
+
 int orc_set_tau0(orc_grid* g, double tau0) {
   if (!g || !(tau0 >= 0.5)) return ORC_EINVAL;
   g->cfg.tau0 = tau0;

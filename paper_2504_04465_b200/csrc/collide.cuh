@@ -17,6 +17,7 @@ struct ModelParams {
   int newton_max_iter, trace_eq;
   int bc_kind[4];
   double bc_rho[4], bc_ux[4], bc_uy[4], bc_T[4];
+  double sponge_rho_inf;
 };
 
 enum { FLAG_UNSTABLE = 1, FLAG_NEWTON = 2 };

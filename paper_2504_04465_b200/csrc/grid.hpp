@@ -31,6 +31,7 @@ struct HostLevel {
   // regular bricks (compressed addressing of the CUDA path): aligned 8x8 tiles of FLUID cells whose
   // every link is reproduced by tile arithmetic.  brick_nb[9*b + k]: storage index of the first cell of the tile at
   // offset (k%3-1, k/3-1) (k = 4: the brick itself).  irr: the cells outside bricks, ascending.
+  std::vector<double> sigma;          // sponge coefficient per stored cell (Eq. 11); empty when no cell of the level has one
   int64_t nbrick = 0;
   std::vector<int32_t> brick_nb;
   std::vector<int32_t> irr;

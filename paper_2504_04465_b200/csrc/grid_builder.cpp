@@ -13,6 +13,7 @@
 #include "grid.hpp"
 
 #include <algorithm>
+#include <cmath>
 #include <atomic>
 #include <cstring>
 #include <new>
@@ -420,6 +421,25 @@ int build_grid(const lbm_config& cfg, const int64_t* split_off, const int32_t* s
     }
     L.ng = (int64_t)L.g_coarse.size();
   }
+  // ---- sponge coefficient of Eq. 11 (reading S24) at the cell centres ((ix+1/2)h, (iy+1/2)h), h = 2^l
+  if (cfg.sponge_sigma_max > 0.0)
+    for (int l = 0; l <= d; ++l) {
+      HostLevel& L = G.lv[l];
+      const double h = (double)((int64_t)1 << l);
+      std::vector<double> sg((size_t)L.n, 0.0);
+      bool any = false;
+      for (int64_t c = 0; c < L.n; ++c) {
+        const double dx = (L.ix[c] + 0.5) * h - cfg.sponge_x0, dy = (L.iy[c] + 0.5) * h - cfg.sponge_y0;
+        const double r = std::sqrt(dx * dx + dy * dy);
+        double v = 0.0;
+        if (r >= cfg.sponge_r1) v = cfg.sponge_sigma_max;
+        else if (r >= cfg.sponge_r0) v = cfg.sponge_sigma_max * (r - cfg.sponge_r0) / (cfg.sponge_r1 - cfg.sponge_r0);
+        sg[(size_t)c] = v;
+        any = any || v > 0.0;
+      }
+      if (any) L.sigma.swap(sg);
+    }
+
   // ---- (9) regular bricks: an aligned 8x8 tile whose 64 cells are stored (hence consecutive along the Z-curve), all
   // FLUID, and whose every list entry equals base[tile of the source] + Z-position of the
   // source inside that tile.  Each candidate is VERIFIED against the list built above, entry by entry, so the
@@ -445,7 +465,8 @@ int build_grid(const lbm_config& cfg, const int64_t* split_off, const int32_t* s
         if (b.cells.bm.word[t] != ~0ull) continue;
         const int32_t base = b.cells.base[t];
         bool ok = true;
-        for (int m = 0; m < 64 && ok; ++m) ok = L.type[(size_t)base + m] == LBM_FLUID;
+        for (int m = 0; m < 64 && ok; ++m)
+          ok = L.type[(size_t)base + m] == LBM_FLUID && (L.sigma.empty() || L.sigma[(size_t)base + m] == 0.0);   // sponge cells use the list path
         if (!ok) continue;
         const int tx = (int)gather_bits((uint64_t)t), ty = (int)gather_bits((uint64_t)t >> 1);
         int32_t* nb = &cand[(size_t)t * 9];

@@ -25,7 +25,8 @@ constexpr size_t ALIGN = 256;
 struct DevLevel {
   int64_t n = 0, ps = 0, ng = 0;
   size_t off_type = 0, off_aux = 0, off_nbr = 0, off_gcoarse = 0, off_gchild = 0, off_S[2] = {0, 0};
-  size_t off_bricks = 0, off_irr = 0;
+  size_t off_bricks = 0, off_irr = 0, off_sigma = 0;
+  double* sigma = nullptr;
   int64_t nbrick = 0, n_irr = 0;
   int* brick_nb = nullptr;
   int* irr = nullptr;
@@ -147,6 +148,7 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   a.fps = l > 0 ? g->dl[l - 1].ps : 0;
   a.tau = g->hg.lv[l].tau;
   a.status = g->d_status;
+  a.sigma = L.sigma;
   a.brick_nb = L.brick_nb; a.brick_tab = g->d_tab; a.irr = L.irr;
   a.nbrick = (int)L.nbrick; a.n_irr = (int)L.n_irr;
   const int64_t cells_per_cta = g->ks->brick_cells_per_cta;
@@ -226,6 +228,10 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
   if (cfg->collision < LBM_BGK || cfg->collision > LBM_NUMEQ) return LBM_EINVAL;
   if (cfg->collision == LBM_RR && cfg->ddf) return LBM_EINVAL;     // RR is defined for the athermal models only
   if (!(cfg->tau0 >= 0.5)) return LBM_EINVAL;
+  // the sponge relaxes rho = p / T0: weakly compressible models only
+  if (cfg->sponge_sigma_max != 0.0 && (cfg->ddf || cfg->collision == LBM_NUMEQ || !(cfg->sponge_sigma_max > 0.0) ||
+                                       !(cfg->sponge_sigma_max <= 1.0) || !(cfg->sponge_r1 > cfg->sponge_r0) || !(cfg->sponge_r0 >= 0.0)))
+    return LBM_EINVAL;
   // velocity bounce-back is defined for the weakly compressible models only
   for (int s = 0; s < 4; ++s)
     if ((cfg->bc[s] == LBM_BC_MOVING_WALL || cfg->bc[s] == LBM_BC_INFLOW_VBB) && (cfg->ddf || cfg->collision == LBM_NUMEQ))
@@ -247,6 +253,7 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
     ModelParams& mp = g->mp;
     mp.gamma = cfg->gamma; mp.sensor_A = cfg->sensor_A; mp.T0 = cfg->T0; mp.newton_tol = cfg->newton_tol;
     mp.newton_max_iter = cfg->newton_max_iter; mp.trace_eq = cfg->trace_eq;
+    mp.sponge_rho_inf = cfg->sponge_rho_inf;
     for (int s = 0; s < 4; ++s) {
       mp.bc_kind[s] = cfg->bc[s];
       mp.bc_rho[s] = cfg->bc_rho[s]; mp.bc_ux[s] = cfg->bc_ux[s]; mp.bc_uy[s] = cfg->bc_uy[s]; mp.bc_T[s] = cfg->bc_T[s];
@@ -269,6 +276,7 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
       L.nbrick = H.nbrick; L.n_irr = (int64_t)H.irr.size();
       L.off_bricks = off; off += round_up((size_t)std::max<int64_t>(H.nbrick, 1) * 36, ALIGN);
       L.off_irr = off; off += round_up((size_t)std::max<int64_t>(L.n_irr, 1) * 4, ALIGN);
+      L.off_sigma = off; off += round_up(H.sigma.size() * 8, ALIGN);
       for (int b = 0; b < 2; ++b) { L.off_S[b] = off; off += round_up((size_t)L.ps * (size_t)g->npop * (size_t)g->esize, ALIGN); }
       g->n_total += H.n;
       nmax = std::max(nmax, H.n);
@@ -358,6 +366,13 @@ int lbm_get_bricks(const lbm_grid* g, int l, int32_t* tiles9, uint16_t* table) {
   return LBM_OK;
 }
 
+int lbm_get_sponge(const lbm_grid* g, int l, double* sigma) {
+  if (!g || !sigma || l < 0 || l > g->depth) return LBM_EINVAL;
+  const HostLevel& H = g->hg.lv[l];
+  for (int64_t c = 0; c < H.n; ++c) sigma[c] = H.sigma.empty() ? 0.0 : H.sigma[(size_t)c];
+  return LBM_OK;
+}
+
 int lbm_get_schedule(const lbm_grid* g, int32_t* k_of, int32_t* level_of, int cap) {
   if (!g) return LBM_EINVAL;
   int n = 0;
@@ -413,6 +428,8 @@ int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream
     L.irr = (int*)(g->arena + L.off_irr);
     if (H.nbrick > 0) CK(cudaMemcpyAsync(L.brick_nb, H.brick_nb.data(), (size_t)H.nbrick * 36, cudaMemcpyHostToDevice, g->stream));
     if (!H.irr.empty()) CK(cudaMemcpyAsync(L.irr, H.irr.data(), H.irr.size() * 4, cudaMemcpyHostToDevice, g->stream));
+    L.sigma = H.sigma.empty() ? nullptr : (double*)(g->arena + L.off_sigma);
+    if (L.sigma) CK(cudaMemcpyAsync(L.sigma, H.sigma.data(), H.sigma.size() * 8, cudaMemcpyHostToDevice, g->stream));
     if (H.ng > 0) {
       CK(cudaMemcpyAsync(L.g_coarse, H.g_coarse.data(), (size_t)H.ng * 4, cudaMemcpyHostToDevice, g->stream));
       CK(cudaMemcpyAsync(L.g_child, H.g_child.data(), (size_t)H.ng * 16, cudaMemcpyHostToDevice, g->stream));

@@ -37,6 +37,7 @@ struct LevelArgs {
   void* fine;               // finer level's CURRENT buffer (coalescence reads, explosion writes)
   long long fps;            // its plane stride
   double tau;
+  const double* sigma;      // sponge coefficient per cell (Eq. 11) or null
   int* status;              // sticky FLAG_* word
   // compressed addressing (BRICKS kernels): the first list_ctas CTAs update the n_irr irregular cells irr[] through the
   // list (first, so that the slower one-cell-per-thread work is not the tail of the launch), the following brick_ctas
@@ -343,6 +344,30 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
       } else {
 #pragma unroll
         for (int k = 0; k < NLAMBDA; ++k) lam[j][k] = So[(PL::L0 + k) * ps + self[j]];
+      }
+    }
+
+    // ---- pressure relaxation of the sponge (Eq. 10, "applied before the collision step" P:303; reading S24):
+    // rho -> rho' = rho (1 - sigma) + sigma rho_inf at unchanged velocity and non-equilibrium part, i.e.
+    // f_i += (rho'/rho - 1) f_i^eq(rho, u); a Neumann cell follows its source (S13).  Sponge cells are never in bricks.
+    if constexpr (!DDF && !NUMEQ) {
+      if (a.sigma != nullptr) {
+        const T sg = T(a.sigma[self[j]]);
+        if (sg > T(0)) {
+          T r = T(0), jx = T(0), jy = T(0);
+          static_for<0, Q>([&](auto ic) {
+            constexpr int I = decltype(ic)::value;
+            constexpr int cx = Lat<Q>::t.cx[I], cy = Lat<Q>::t.cy[I];
+            r += f[j][I];
+            if constexpr (cx != 0) jx += T(cx) * f[j][I];
+            if constexpr (cy != 0) jy += T(cy) * f[j][I];
+          });
+          T ae[NA];
+          aeq_moments<T>(r, jx / r, jy / r, T(0), ae);
+          const T rn = r * (T(1) - sg) + sg * T(p.sponge_rho_inf);
+          const T w = rn / r - T(1);
+          poly_all<Q, T>(ae, [&](auto ic, T fe) { f[j][decltype(ic)::value] += w * fe; });
+        }
       }
     }
 

@@ -23,7 +23,7 @@ _ERR = {EINVAL: "LBM_EINVAL", ENOMEM: "LBM_ENOMEM", EMESH: "LBM_EMESH", ECUDA: "
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
-           "lbm_get_schedule", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic",
+           "lbm_get_schedule", "lbm_get_sponge", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic",
            "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_measure_fma_peak"]
 
 
@@ -41,6 +41,8 @@ class LbmConfig(C.Structure):
         ("tau0", C.c_double), ("T0", C.c_double), ("gamma", C.c_double), ("sensor_A", C.c_double),
         ("newton_tol", C.c_double),
         ("bc_rho", C.c_double * 4), ("bc_ux", C.c_double * 4), ("bc_uy", C.c_double * 4), ("bc_T", C.c_double * 4),
+        ("sponge_x0", C.c_double), ("sponge_y0", C.c_double), ("sponge_r0", C.c_double), ("sponge_r1", C.c_double),
+        ("sponge_sigma_max", C.c_double), ("sponge_rho_inf", C.c_double),
     ]
 
 
@@ -75,6 +77,7 @@ def lib():
         L.lbm_get_ghosts.argtypes = [vp, C.c_int, vp, vp, vp]
         L.lbm_get_schedule.argtypes = [vp, vp, vp, C.c_int]
         L.lbm_get_bricks.argtypes = [vp, C.c_int, vp, vp]
+        L.lbm_get_sponge.argtypes = [vp, C.c_int, vp]
         L.lbm_grid_bind.argtypes = [vp, vp, C.c_size_t, vp]
         L.lbm_init_fields.argtypes = [vp, vp, vp, vp, vp]
         L.lbm_step.argtypes = [vp, C.c_int]
@@ -112,8 +115,12 @@ def _check(where, rc):
 
 def make_config(lattice=9, precision=64, collision=BGK, ddf=0, sensor=0, trace_eq=0, depth=0, nx_coarse=1, ny_coarse=1,
                 tau0=0.6, T0=0.0, gamma=1.4, sensor_A=1.5, newton_tol=1e-12, newton_max_iter=50,
-                bc=(0, 0, 0, 0), bc_rho=(1, 1, 1, 1), bc_ux=(0, 0, 0, 0), bc_uy=(0, 0, 0, 0), bc_T=(0, 0, 0, 0)):
+                bc=(0, 0, 0, 0), bc_rho=(1, 1, 1, 1), bc_ux=(0, 0, 0, 0), bc_uy=(0, 0, 0, 0), bc_T=(0, 0, 0, 0),
+                sponge=None):
+    """sponge: None or (x0, y0, r0, r1, sigma_max, rho_inf) of Eq. 10-11."""
     c = LbmConfig()
+    if sponge is not None:
+        (c.sponge_x0, c.sponge_y0, c.sponge_r0, c.sponge_r1, c.sponge_sigma_max, c.sponge_rho_inf) = [float(v) for v in sponge]
     c.lattice, c.precision, c.collision, c.ddf, c.sensor, c.trace_eq = lattice, precision, collision, ddf, sensor, trace_eq
     c.depth, c.nx_coarse, c.ny_coarse, c.newton_max_iter = depth, nx_coarse, ny_coarse, newton_max_iter
     c.tau0, c.T0, c.gamma, c.sensor_A, c.newton_tol = tau0, T0, gamma, sensor_A, newton_tol
@@ -186,6 +193,11 @@ class Grid:
     def nbr(self, l):
         a = np.zeros((self.n[l], self.Q - 1), np.int32)
         _check("lbm_get_nbr", lib().lbm_get_nbr(self.h, l, _ptr(a)))
+        return a
+
+    def sponge(self, l):
+        a = np.zeros(self.n[l])
+        _check("lbm_get_sponge", lib().lbm_get_sponge(self.h, l, _ptr(a)))
         return a
 
     def bricks(self, l):

@@ -58,6 +58,7 @@ class Case:
     bc_ux: tuple = (0.0, 0.0, 0.0, 0.0)
     bc_uy: tuple = (0.0, 0.0, 0.0, 0.0)
     bc_T: tuple = (0.0, 0.0, 0.0, 0.0)
+    sponge: object = None      # None or (x0, y0, r0, r1, sigma_max, rho_inf): pressure-relaxation sponge, Eq. 10-11
     fields: object = None      # callable(level, ix, iy) -> rho, ux, uy, T  (arrays; centres are (ix+.5)*2^level)
     meta: dict = field(default_factory=dict)
 
@@ -66,7 +67,7 @@ class Case:
                     trace_eq=self.trace_eq, depth=self.mesh.depth, nx_coarse=self.mesh.nx_coarse,
                     ny_coarse=self.mesh.ny_coarse, tau0=self.tau0, T0=self.T0, gamma=self.gamma,
                     sensor_A=self.sensor_A, newton_tol=self.newton_tol, newton_max_iter=self.newton_max_iter,
-                    bc=self.bc, bc_rho=self.bc_rho, bc_ux=self.bc_ux, bc_uy=self.bc_uy, bc_T=self.bc_T)
+                    bc=self.bc, bc_rho=self.bc_rho, bc_ux=self.bc_ux, bc_uy=self.bc_uy, bc_T=self.bc_T, sponge=self.sponge)
 
 
 def empty_levels(depth):
@@ -161,9 +162,11 @@ def cavity(scale=1.0, collision=RR, re=1000.0, u_lid=0.1, trace_eq=0, lattice=9)
 CYL_RADII_D = (6.5, 11.0, 17.0, 23.0, 29.0)   # refinement radii R_0..R_4 in cylinder diameters
 
 
-def cylinder(D=200, depth=5, mach=0.2, re=150.0, seed=1234, collision=RR, lattice=9, radii=CYL_RADII_D):
+def cylinder(D=200, depth=5, mach=0.2, re=150.0, seed=1234, collision=RR, lattice=9, radii=CYL_RADII_D, sponge_d=None):
     """Flow past a circular cylinder of diameter D finest cells in a 64D x 64D box, `depth`+1 levels graded
-    by distance from the cylinder; left inflow (velocity bounce-back), other sides Neumann."""
+    by distance from the cylinder; left inflow (velocity bounce-back), other sides Neumann.
+    sponge_d = (r0, r1, sigma_max) in diameters switches the pressure-relaxation sponge of Eq. 10-11 on around the
+    cylinder centre with rho_inf = 1 (the paper: 130 D, 180 D, 0.1 in a 400 D domain; here e.g. (24, 30, 0.1))."""
     L = 64 * D
     nc = L >> depth
     assert nc << depth == L, "64*D must be divisible by 2^depth"
@@ -192,7 +195,8 @@ def cylinder(D=200, depth=5, mach=0.2, re=150.0, seed=1234, collision=RR, lattic
         uy = u_inf * 1e-4 * hash_uniform(seed, level, ix, iy, 1)
         return o, ux, uy, cs2 * o
 
-    return Case("cylinder", mesh, lattice=lattice, collision=collision, tau0=tau0,
+    sponge = None if sponge_d is None else (cxc, cyc, sponge_d[0] * D, sponge_d[1] * D, sponge_d[2], 1.0)
+    return Case("cylinder", mesh, lattice=lattice, collision=collision, tau0=tau0, sponge=sponge,
                 bc=(BC_INFLOW_VBB, BC_NEUMANN, BC_NEUMANN, BC_NEUMANN), bc_ux=(u_inf, 0, 0, 0), fields=fields,
                 meta=dict(D=D, u_inf=u_inf, re=re, nu0=nu0, mach=mach))
 

@@ -43,6 +43,7 @@ CASES = {
     "cavity": lambda: W.cavity(),
     "cavity_q13": lambda: W.cavity(scale=0.5, lattice=13),
     "cylinder_small": lambda: W.cylinder(D=40, depth=3, radii=(3, 5, 8)),
+    "cylinder_sponge": lambda: W.cylinder(D=40, depth=3, radii=(3, 5, 8), sponge_d=(24, 30, 0.1)),
     "riemann_neumann": lambda: W.riemann(n=64),
     "riemann_periodic": lambda: W.riemann(n=48, periodic=True),
     "naca_small": lambda: W.naca(chord=64, depth=3, radii=(1, 2.5, 5), aoa_deg=4.0),
@@ -65,6 +66,7 @@ def test_host_builder_bit_exact_against_oracle_builder(name):
             assert np.array_equal(a, b)
         assert np.array_equal(g.nbr(l), o.nbr(l))
         assert g.tau(l) == o.tau(l)
+        assert np.array_equal(g.sponge(l), o.sponge(l))          # Eq. 11 at the cell centres, bit for bit
         if l >= 1:
             for a, b in zip(g.ghosts(l), o.ghosts(l)):
                 assert np.array_equal(a, b)
@@ -109,6 +111,7 @@ def test_bricks_reproduce_the_oracle_neighbour_list(name):
         assert np.all(np.diff(base) >= 64)
         cells = base[:, None] + mm[None, :]
         assert np.all(ty[cells] == O.FLUID)
+        assert np.all(o.sponge(l)[cells] == 0.0)                  # sponge cells go through the list path
         assert np.all(ix[base] % 8 == 0) and np.all(iy[base] % 8 == 0)
         x, y = _zpos(mm)
         assert np.array_equal(ix[cells], ix[base][:, None] + x[None, :])

@@ -30,6 +30,7 @@ def _cases():
         "tgv64_rr": (lambda: W.tgv(64, collision=W.RR), 20),
         "cavity": (lambda: W.cavity(), 10),                                     # walls, moving lid, 2 levels
         "cylinder_small": (lambda: W.cylinder(D=40, depth=3, radii=(3, 5, 8)), 3),
+        "cylinder_sponge": (lambda: W.cylinder(D=40, depth=3, radii=(3, 5, 8), sponge_d=(24, 30, 0.1)), 3),   # Eq. 10-11
         "patch_q13": (lambda: W.patch(nc=64, lo=16, hi=48, lattice=13, collision=W.RR, tau0=0.7, fields=_fields(64, 1, 0.5)), 4),
         "patch_q21": (lambda: W.patch(nc=64, lo=16, hi=48, lattice=21, collision=W.BGK, tau0=0.7, fields=_fields(64, 1, 2.0 / 3.0)), 4),
         "riemann_q37_ddf_sensor": (lambda: W.riemann(n=64), 3),                 # Neumann layers; fp64 only (as in test_gpu_parity)

@@ -268,3 +268,24 @@ def test_mach_ramp_on_dirichlet_sides_naca():
     assert g.sync() == 0
     assert max_pop_diff(g, o, (0, 1)) <= 1e-12
     g.close()
+
+
+# ------------------------------------------------------------------ pressure-relaxation sponge (Eq. 10-11; S24)
+@pytest.mark.parametrize("precision", [64, 32])
+def test_sponge_uniform_relaxation_and_cylinder(precision):
+    """The sponge in the kernels against the oracle: a uniform box away from rho_inf (every cell at sigma_max: the
+    geometric relaxation of tests/test_oracle_sponge.py) and the scaled cylinder with the outer ring of Eq. 11."""
+    tol = 1e-12 if precision == 64 else 1e-5
+    sp = (8.0, 8.0, 1e-9, 2e-9, 0.1, 1.0)
+
+    def fields(level, ix, iy):
+        o = np.ones(len(ix))
+        return 1.2 * o, 0.05 * o, -0.02 * o, o / 3.0
+    box = W.Case("uniform", W.uniform_mesh(24, 24), collision=W.RR, tau0=0.7, bc=(W.BC_PERIODIC,) * 4, fields=fields, sponge=sp)
+    g, o, d0 = run_pair(box, precision, 10)
+    assert max_pop_diff(g, o) <= tol
+    assert abs(g.macroscopic()[0].mean() - (1.0 + 0.9 ** 10 * 0.2)) < (1e-12 if precision == 64 else 1e-5)
+    g.close()
+    g, o, d0 = run_pair(W.cylinder(D=40, depth=3, radii=(3, 5, 8), sponge_d=(24, 30, 0.1)), precision, 4)
+    assert max_pop_diff(g, o) <= tol
+    g.close()
