@@ -15,7 +15,7 @@
  * gathers f*_i(x-xi_i,t) (pull form of Eq. 31), then collides.
  *
  * Parity status of each part is listed in DESIGN.md ("Pins"); long-run fields of the
- * cylinder / Riemann / NACA workloads are "parity unpinned" beyond GPU-vs-oracle.
+ * 2-D Riemann / NACA workloads are "parity unpinned" beyond GPU-vs-oracle.
  */
 #ifndef ORACLE_H
 #define ORACLE_H

@@ -1,0 +1,47 @@
+"""A physical result of the CUDA path at scale against a value the PAPER prints (not against the oracle): the Strouhal
+number of the vortex street behind the cylinder of configs[2] at (Re, Ma) = (150, 0.2), St = 0.1824 in the paper, 0.183 in
+the DNS it cites, 0.179-0.185 in experiments (tests/golden/strouhal_aeolian.txt).  Half-resolution copy of the bench
+workload (D = 100 finest cells, 6 levels, 2.5 M cells, inflow / Neumann / bounce-back links, every interface, the sponge of
+Eq. 10-11) run for 400 convective times = 346 k fine steps (~25 s on a B200; the oracle would need a week), cross-stream
+velocity probed two diameters behind the cylinder, spectrum by FFT with a Hamming window and zero padding as in P:317."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2504_04465_b200 import lbm, workloads as W
+
+pytestmark = pytest.mark.gpu
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "strouhal_aeolian.txt")
+
+
+def test_cylinder_wake_strouhal_number_matches_the_paper():
+    gold = {l.split()[0]: float(l.split()[1]) for l in open(GOLD) if l.strip() and not l.startswith("#")}
+    D, every, t_total = 100, 8, 400.0
+    case = W.cylinder(D=D, sponge_d=(24, 30, 0.1))
+    g = lbm.Grid.from_case(case, precision=64).bind("cuda:0")
+    cells = [g.cells(l)[:2] for l in range(g.depth + 1)]
+    assert g.init_fields(*W.eval_fields(case, cells)) == 0
+    u_inf = case.meta["u_inf"]
+    tc = D / u_inf                                     # fine steps per convective time D / u_inf
+    fine_per_coarse = 1 << g.depth
+    ix, iy = cells[0]
+    L = 64 * D
+    probe = int(np.argmin((ix + 0.5 - (L / 2 + 2.0 * D)) ** 2 + (iy + 0.5 - L / 2) ** 2))
+    t, v = [], []
+    for s in range(0, int(t_total * tc / fine_per_coarse), every):
+        g.step(every)
+        v.append(g.macroscopic()[2][probe])            # level 0 comes first in the flat arrays
+        t.append((s + every) * fine_per_coarse)
+    assert g.sync() == 0                               # stable for 400 convective times
+    g.close()
+    t, v = np.array(t, float), np.array(v)
+    n0 = int(0.6 * len(t))                             # the shedding has saturated by ~120 t_c
+    sig = v[n0:] - v[n0:].mean()
+    assert np.abs(sig).max() > 0.3 * u_inf             # a fully developed street: v' of the order of u_inf at the probe
+    npad = 16 * len(sig)
+    spec = np.abs(np.fft.rfft(sig * np.hamming(len(sig)), npad))
+    freq = np.fft.rfftfreq(npad, d=t[1] - t[0])
+    st = freq[spec[1:].argmax() + 1] * D / u_inf
+    assert gold["experiment_lo"] <= st <= gold["experiment_hi"], st
+    assert abs(st - gold["paper_lbm"]) < 0.003, st     # measured 0.1830 (fp64) / 0.1833 (fp32); DNS 0.183
