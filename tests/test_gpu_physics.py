@@ -45,3 +45,29 @@ def test_cylinder_wake_strouhal_number_matches_the_paper():
     st = freq[spec[1:].argmax() + 1] * D / u_inf
     assert gold["experiment_lo"] <= st <= gold["experiment_hi"], st
     assert abs(st - gold["paper_lbm"]) < 0.003, st     # measured 0.1830 (fp64) / 0.1833 (fp32); DNS 0.183
+
+
+@pytest.mark.parametrize("lattice,precision", [(13, 64), (21, 64), (37, 64), (21, 32)])
+def test_sod_shock_tube_on_the_gpu_matches_the_exact_riemann_solution(lattice, precision):
+    """The numerical-equilibrium + g + sensor kernels on the Sod tube of Eq. 12 at N = 1024 (an order of magnitude
+    beyond what the oracle pin of tests/test_oracle_sod.py runs) against the exact solution of the Euler Riemann problem:
+    first-order convergence carries the oracle's 0.9 % L1 density error at N = 256 down to ~0.25 %."""
+    from test_oracle_sod import GAMMA, exact_riemann_density
+    N = 1024
+    case = W.sod(L=N, lattice=lattice, mesh="unif", periodic=False, ny=16)
+    g = lbm.Grid.from_case(case, precision=precision).bind("cuda:0")
+    cells = [g.cells(0)[:2]]
+    assert g.init_fields(*W.eval_fields(case, cells)) == 0
+    nsteps = int(round(0.2 * N / np.sqrt(GAMMA * W.SOD_T0[lattice])))
+    g.step(nsteps)
+    assert g.sync() == 0
+    rho = g.macroscopic()[0]
+    g.close()
+    ix, iy = cells[0]
+    m = (iy == 7) & (ix >= 0) & (ix < N)
+    order = np.argsort(ix[m])
+    x = ix[m][order] + 0.5
+    (rl, _, Tl), (rr, _, Tr) = case.meta["left"], case.meta["right"]
+    exact, _ = exact_riemann_density((x - N / 2) / nsteps, (rl, 0.0, rl * Tl), (rr, 0.0, rr * Tr))
+    err = float(np.abs(rho[m][order] - exact).sum() / np.abs(exact).sum())
+    assert err < 0.004, err
