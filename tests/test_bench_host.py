@@ -77,3 +77,26 @@ def test_moved_bytes_count_bricks_only_on_large_levels():
     big = lbm.Grid.from_case(W.tgv(1024))
     assert bench.moved_bytes_per_update(big, W.tgv(1024), 64) == pytest.approx(144 + 36 / 64)
     small.close(); big.close()
+
+
+def test_byte_accounting_reproduces_the_papers_list_penalty_table():
+    """Eq. 14-16: a matrix-like update moves 2 n s + 8 B per cell, the tree adds (Q-1) 4 B of neighbour list; the
+    ratios of Table 1 (golden fixture) follow, and bench.py's list-addressed figure is the tree's minus the 4 B own index that
+    a pull kernel does not read."""
+    import bench
+    from paper_2504_04465_b200 import workloads as W
+    gold = {}
+    for line in open(os.path.join(ROOT, "tests", "golden", "table1_list_penalty.txt")):
+        if line.strip() and not line.startswith("#"):
+            c = line.split()
+            gold[(c[0], c[1])] = [float(x) for x in c[2:]]
+    for (model, prec), ratios in gold.items():
+        s = 4 if prec == "sp" else 8
+        for Q, r in zip((9, 13, 21, 37), ratios):
+            n = Q if model == "weakly" else 2 * Q + 8
+            matrix, tree = 2 * n * s + 8, 2 * n * s + 8 + (Q - 1) * 4
+            assert abs(matrix / tree - r) < 0.0051, (model, prec, Q, matrix / tree, r)
+    for prec, s in ((64, 8), (32, 4)):
+        assert bench.algorithmic_bytes_per_update(W.tgv(64), prec) == 2 * 9 * s + 8 + 8 * 4 - 4
+    naca = W.naca(chord=64, depth=3, radii=(1, 2.5, 5))
+    assert bench.algorithmic_bytes_per_update(naca, 64) == 2 * (2 * 21 + 8) * 8 + 8 + 20 * 4 - 4
