@@ -280,7 +280,7 @@ __device__ __forceinline__ bool newton_direction(const T (&f)[Q], const T (&G)[N
       A[i][j] = t * rd[j];
     });
   });
-  T z[NLAMBDA];
+  T z[NLAMBDA] = {};
   static_for<0, NLAMBDA>([&](auto ic) {          // L z = G
     constexpr int i = decltype(ic)::value;
     T t = G[i];

@@ -24,33 +24,26 @@ namespace lbm {
 // ------------------------------------------------------------------ lattices (Table 4)
 bool make_lattice(int Q, Lattice* L) {
   struct Group { int a, b; double w; };
-  std::vector<Group> groups;
+  static const Group g9[] = {{0, 0, 4.0 / 9.0}, {1, 0, 1.0 / 9.0}, {1, 1, 1.0 / 36.0}};
+  static const Group g13[] = {{0, 0, 3.0 / 8.0}, {1, 0, 1.0 / 12.0}, {1, 1, 1.0 / 16.0}, {2, 0, 1.0 / 96.0}};
+  static const Group g21[] = {{0, 0, 91.0 / 324.0}, {1, 0, 1.0 / 12.0}, {1, 1, 2.0 / 27.0}, {2, 0, 7.0 / 360.0},
+                              {2, 2, 1.0 / 432.0}, {3, 0, 1.0 / 1620.0}};
+  static const Group g37[] = {{0, 0, 0.233150669132352}, {1, 0, 0.107306091542219}, {1, 1, 0.057667859888794},
+                              {2, 0, 0.014208216158450}, {2, 1, 0.005353049000513}, {2, 2, 0.001011937592673},
+                              {3, 0, 0.000245301027757}, {3, 1, 0.000283414252994}};
+  const Group* groups = nullptr;
+  int ngroups = 0;
   switch (Q) {
-    case 9:
-      groups = {{0, 0, 4.0 / 9.0}, {1, 0, 1.0 / 9.0}, {1, 1, 1.0 / 36.0}};
-      L->cs2 = 1.0 / 3.0;
-      break;
-    case 13:
-      groups = {{0, 0, 3.0 / 8.0}, {1, 0, 1.0 / 12.0}, {1, 1, 1.0 / 16.0}, {2, 0, 1.0 / 96.0}};
-      L->cs2 = 0.5;
-      break;
-    case 21:
-      groups = {{0, 0, 91.0 / 324.0}, {1, 0, 1.0 / 12.0}, {1, 1, 2.0 / 27.0}, {2, 0, 7.0 / 360.0},
-                {2, 2, 1.0 / 432.0}, {3, 0, 1.0 / 1620.0}};
-      L->cs2 = 2.0 / 3.0;
-      break;
-    case 37:
-      groups = {{0, 0, 0.233150669132352}, {1, 0, 0.107306091542219}, {1, 1, 0.057667859888794},
-                {2, 0, 0.014208216158450}, {2, 1, 0.005353049000513}, {2, 2, 0.001011937592673},
-                {3, 0, 0.000245301027757}, {3, 1, 0.000283414252994}};
-      L->cs2 = 0.697953322019683;
-      break;
-    default:
-      return false;
+    case 9: groups = g9; ngroups = 3; L->cs2 = 1.0 / 3.0; break;
+    case 13: groups = g13; ngroups = 4; L->cs2 = 0.5; break;
+    case 21: groups = g21; ngroups = 6; L->cs2 = 2.0 / 3.0; break;
+    case 37: groups = g37; ngroups = 8; L->cs2 = 0.697953322019683; break;
+    default: return false;
   }
   int n = 0, reach = 0;
   auto put = [&](int x, int y, double w) { L->cx[n] = x; L->cy[n] = y; L->w[n] = w; ++n; };
-  for (const Group& g : groups) {
+  for (int gi = 0; gi < ngroups; ++gi) {
+    const Group& g = groups[gi];
     const int a = g.a, b = g.b;
     reach = std::max(reach, std::max(a, b));
     if (a == 0) {
