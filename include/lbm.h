@@ -170,6 +170,10 @@ int lbm_sync(lbm_grid* g);
 /* rho, u (and T by Eq. 51) of every stored cell from its current populations; HOST outputs of
  * n_total doubles, any may be NULL.  Synchronises. */
 int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double* T);
+/* The same for n probe cells of one level (storage indices in `cells`, HOST int32): time series without moving the whole
+ * field (the steady-state, Strouhal and pressure-probe post-processing of Sec. 5 needs a few cells every few steps).
+ * HOST outputs of n doubles, any may be NULL.  Synchronises.  LBM_EINVAL for an index outside the level. */
+int lbm_get_macroscopic_at(lbm_grid* g, int level, int n, const int32_t* cells, double* rho, double* ux, double* uy, double* T);
 /* Current populations of one level as HOST doubles, row-major [cell][component];
  * which: 0 = f (Q), 1 = g (Q), 2 = lambda (8).  Synchronises. */
 int lbm_get_populations(lbm_grid* g, int level, int which, double* out);

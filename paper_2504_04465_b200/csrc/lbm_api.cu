@@ -604,7 +604,7 @@ int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double
   for (int l = 0; l <= g->depth; ++l) {
     DevLevel& L = g->dl[l];
     MacroArgs a;
-    a.n = (int)L.n; a.ps = L.ps; a.S = L.S[L.cur];
+    a.n = (int)L.n; a.ps = L.ps; a.S = L.S[L.cur]; a.cells = nullptr;
     a.rho = d[0] + base; a.ux = d[1] + base; a.uy = d[2] + base; a.Tm = d[3] + base;
     int rc = launch(g->ks->macro, L.n, &a, &g->mp, g->stream);
     if (rc) return rc;
@@ -613,6 +613,29 @@ int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double
   double* h[4] = {rho, ux, uy, T};
   for (int k = 0; k < 4; ++k)
     if (h[k]) CK(cudaMemcpyAsync(h[k], d[k], N * 8, cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return LBM_OK;
+}
+
+int lbm_get_macroscopic_at(lbm_grid* g, int l, int n, const int32_t* cells, double* rho, double* ux, double* uy, double* T) {
+  if (!g || !cells || n < 0 || l < 0 || l > g->depth) return LBM_EINVAL;
+  if (!g->bound || !g->inited) return LBM_ESTATE;
+  if (n == 0) return LBM_OK;
+  DevLevel& L = g->dl[l];
+  if ((size_t)n * 5 + 8 > g->scratch_doubles) return LBM_EINVAL;
+  for (int k = 0; k < n; ++k)
+    if (cells[k] < 0 || cells[k] >= L.n) return LBM_EINVAL;
+  double* d[4] = {g->d_scratch, g->d_scratch + n, g->d_scratch + 2 * (size_t)n, g->d_scratch + 3 * (size_t)n};
+  int* d_cells = (int*)(g->d_scratch + 4 * (size_t)n);
+  CK(cudaMemcpyAsync(d_cells, cells, (size_t)n * 4, cudaMemcpyHostToDevice, g->stream));
+  MacroArgs a;
+  a.n = n; a.ps = L.ps; a.S = L.S[L.cur]; a.cells = d_cells;
+  a.rho = d[0]; a.ux = d[1]; a.uy = d[2]; a.Tm = d[3];
+  int rc = launch(g->ks->macro, n, &a, &g->mp, g->stream);
+  if (rc) return rc;
+  double* h[4] = {rho, ux, uy, T};
+  for (int k = 0; k < 4; ++k)
+    if (h[k]) CK(cudaMemcpyAsync(h[k], d[k], (size_t)n * 8, cudaMemcpyDeviceToHost, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   return LBM_OK;
 }

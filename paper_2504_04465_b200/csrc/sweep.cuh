@@ -562,6 +562,7 @@ struct MacroArgs {
   int n;
   long long ps;
   const void* S;
+  const int* cells;         // probe list (lbm_get_macroscopic_at): output t is cell cells[t]; null: output t is cell t
   double* rho; double* ux; double* uy; double* Tm;
 };
 
@@ -569,8 +570,9 @@ template <int Q, typename T, int COLL, bool DDF>
 __global__ void __launch_bounds__(128) macroscopic_kernel(const MacroArgs a, const ModelParams p) {
   using PL = PopLayout<Q, DDF, COLL>;
   constexpr bool THERMAL = (COLL == LBM_NUMEQ) || DDF;
-  const int c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= a.n) return;
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= a.n) return;
+  const int c = a.cells ? a.cells[t] : t;
   const T* S = (const T*)a.S;
   T f[Q], g[Q];
 #pragma unroll
@@ -581,7 +583,7 @@ __global__ void __launch_bounds__(128) macroscopic_kernel(const MacroArgs a, con
   }
   T rho, ux, uy, Tm;
   moments<Q, T, THERMAL, DDF>(p, f, g, rho, ux, uy, Tm);
-  a.rho[c] = (double)rho; a.ux[c] = (double)ux; a.uy[c] = (double)uy; a.Tm[c] = (double)Tm;
+  a.rho[t] = (double)rho; a.ux[t] = (double)ux; a.uy[t] = (double)uy; a.Tm[t] = (double)Tm;
 }
 
 // ------------------------------------------------------------------ dispatch table entry

@@ -289,3 +289,24 @@ def test_sponge_uniform_relaxation_and_cylinder(precision):
     g, o, d0 = run_pair(W.cylinder(D=40, depth=3, radii=(3, 5, 8), sponge_d=(24, 30, 0.1)), precision, 4)
     assert max_pop_diff(g, o) <= tol
     g.close()
+
+
+def test_probe_cells_agree_with_the_full_field():
+    """lbm_get_macroscopic_at returns, for any list of storage indices of a level, exactly what lbm_get_macroscopic returns
+    for those cells; indices outside the level are rejected."""
+    from paper_2504_04465_b200 import lbm
+    case = W.cavity(scale=0.25)
+    g = gpu_from_case(case, 64)
+    g.step(5)
+    full = g.macroscopic()
+    off = 0
+    rng = np.random.default_rng(3)
+    for l in range(g.depth + 1):
+        idx = rng.integers(0, g.n[l], size=257)
+        got = g.macroscopic_at(l, idx)
+        for k in range(4):
+            assert np.array_equal(got[k], full[k][off + idx])
+        off += g.n[l]
+    with pytest.raises(lbm.LbmError):
+        g.macroscopic_at(0, [g.n[0]])
+    g.close()

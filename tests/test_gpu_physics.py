@@ -31,7 +31,7 @@ def test_cylinder_wake_strouhal_number_matches_the_paper():
     t, v = [], []
     for s in range(0, int(t_total * tc / fine_per_coarse), every):
         g.step(every)
-        v.append(g.macroscopic()[2][probe])            # level 0 comes first in the flat arrays
+        v.append(g.macroscopic_at(0, [probe])[2][0])   # one probe cell, not the whole field
         t.append((s + every) * fine_per_coarse)
     assert g.sync() == 0                               # stable for 400 convective times
     g.close()
