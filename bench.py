@@ -371,12 +371,16 @@ def main():
     # counters of the dominant kernel (finest level's sweep) from the committed ncu --set full captures
     traffic = traffic_src = None
     counters = {}
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tp):
         try:
-            counters = json.load(open(tp)).get("%s_f%d" % (args.workload, args.precision)) or {}
+            import csv
+            rows = {r["key"]: r for r in csv.DictReader(open(tp))}
+            r = rows.get("%s_f%d" % (args.workload, args.precision))
+            if r:
+                counters = {k: (float(v) if k not in ("key", "source") else v) for k, v in r.items() if v != ""}
             if args.scale == 1.0 and int(counters.get("cells_per_launch", -1)) == int(g.n[0]):
-                traffic, traffic_src = counters["bytes_per_launch"], counters["source"]
+                traffic, traffic_src = int(counters["bytes_per_launch"]), counters["source"]
         except Exception:
             counters = {}
     # ALU-bound path (numerical equilibria): fp64 flop per update from the ncu capture against the FMA peak measured now
@@ -386,7 +390,7 @@ def main():
         tf = upd * K * counters["fp64_flop_per_update"] / (ms * 1e-3) / 1e12
         alu = {"bound": "alu", "achieved": tf, "peak": fma_peak, "unit": "TFLOP/s", "frac": tf / fma_peak, "traffic": traffic,
                "peak_source": "lbm_measure_fma_peak(64) measured in this run (148 SMs x 64 fp64 FMA lanes x clock)",
-               "flop_per_update": counters["fp64_flop_per_update"], "flop_source": counters.get("fp64_note"),
+               "flop_per_update": counters["fp64_flop_per_update"], "flop_source": "profiles/traffic.md",
                "fp64_pipe_pct_ncu": counters.get("fp64_pipe_pct")}
     n_all = ntot
     depth = g.depth
