@@ -63,7 +63,7 @@ constexpr int cells_per_thread = (sizeof(T) == 4 && !DDF && COLL != LBM_NUMEQ &&
 
 // Resident CTAs per SM asked of ptxas (register cap): D2Q9 runs at 8 x 128 threads (64 registers).
 template <int Q, typename T, int COLL, bool DDF>
-constexpr int min_ctas_per_sm = (Q == 9 && !DDF && COLL != LBM_NUMEQ) ? 8 : (COLL == LBM_NUMEQ && sizeof(T) == 4 && Q == 13) ? 4 : 1;
+constexpr int min_ctas_per_sm = (Q == 9 && !DDF && COLL != LBM_NUMEQ) ? 8 : (COLL == LBM_NUMEQ && sizeof(T) == 4 && Q == 13) ? 5 : 1;
 
 template <typename T, int N> struct alignas(sizeof(T) * N) Vec { T v[N]; };
 
