@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the quadtree-LBM hot path on B200 (contract: one JSON line on stdout, rank 0).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--precision 64|32]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--precision 64|32] [--addressing auto|list|bricks]
     python bench.py --impl reference ...          # the CPU oracle as it stands, timed on the host cores
 
 A "step" is one pass of the whole hot path over the workload: one COARSE step = 2^depth fine steps of the
@@ -15,10 +15,14 @@ Workloads (synthetic, seeded, shaped like the paper's cases):
   cylinder  BASELINE configs[2]: D2Q9-RR, 6 levels, ~9.85 M cells (default: the multilevel headline)
   uniform   configs[0] scaled to 4096^2 (tree-stored uniform periodic D2Q9-BGK; the 80 %-of-HBM target)
   cavity    configs[1] as given (39 k cells, launch-latency-bound)    cavity8: the same x8
-  riemann   configs[3]: D2Q37 polynomial + g + sensor, 2048^2
+  riemann   configs[3]: D2Q37 polynomial + g + sensor, 2048^2        riemann:numeq: the same box with the numerical equilibrium
   naca      configs[4]: D2Q21 numerical equilibrium + g + sensor, 7 levels, ~18 M cells
+  sod:<Q>:<mesh>  Table 3 of the paper (numerical equilibrium + g + sensor, single precision there)
+The default line also measures the other configs briefly (`also`), each with its own roofline block.
 """
 import argparse
+import csv
+import hashlib
 import json
 import os
 import subprocess
@@ -40,6 +44,10 @@ PAPER_TABLE3 = {(13, "unif"): 1259.1, (13, "hori"): 1088.4, (13, "band"): 1244.8
                 (37, "unif"): 286.9, (37, "hori"): 263.0, (37, "band"): 307.4, (37, "sqr"): 266.1}
 REFERENCE_BUDGET_S = 180     # wall-clock cap of the timed region of --impl reference
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
+ADDRESSING = {"auto": 0, "list": 1, "bricks": 2}      # lbm_config.addressing (LBM_ADDR_*)
+# other workloads measured briefly into the default line's `also` (name[@f32|@f64][@list|@bricks])
+DEFAULT_ALSO = "cavity,uniform,cylinder@list,riemann,naca,sod:21:unif@f32"
+KERNEL_SOURCES = ("lattice.cuh", "collide.cuh", "sweep.cuh")
 
 
 def make_case(name, scale):
@@ -65,9 +73,13 @@ def make_case(name, scale):
     if name == "riemann":
         n = int(round(2048 * scale))
         return W.riemann(n=n), dict(workload="riemann (BASELINE configs[3]): D2Q37 polynomial+g+sensor, %d^2, Neumann box" % n, steps=200)
+    if name == "riemann:numeq":       # configs[3]'s box with the model the paper runs on D2Q37: stable for the 2000 steps
+        n = int(round(2048 * scale))
+        return W.riemann(n=n, collision=W.NUMEQ), dict(
+            workload="riemann:numeq (BASELINE configs[3] box, 2000 steps): D2Q37 numerical eq.+g+sensor, %d^2, Neumann box" % n, steps=2000)
     if name == "naca":
         c = int(round(1024 * scale))
-        return W.naca(chord=c), dict(workload="naca (BASELINE configs[4]): D2Q21 numerical eq.+g+sensor, chord %d, 7 levels" % c, steps=8)
+        return W.naca(chord=c), dict(workload="naca (BASELINE configs[4]): D2Q21 numerical eq.+g+sensor, chord %d, 7 levels" % c, steps=8, also_steps=2)
     if name.startswith("sod"):
         # sod[:lattice[:mesh]], e.g. sod:21:unif -- the paper's only absolute GPU figures (Table 3a)
         parts = name.split(":")
@@ -80,12 +92,14 @@ def make_case(name, scale):
     raise SystemExit("unknown workload %r" % name)
 
 
+def npop_of(case):
+    return case.lattice * (2 if case.ddf else 1) + (8 if case.collision == W.NUMEQ else 0)
+
+
 def algorithmic_bytes_per_update(case, precision):
     """Two-buffer pull update with an int32 list and a type byte:
     2*npop*s + (Q-1)*4 + 4 per cell update."""
-    Q = case.lattice
-    npop = Q * (2 if case.ddf else 1) + (8 if case.collision == W.NUMEQ else 0)
-    return 2 * npop * (precision // 8) + (Q - 1) * 4 + 4
+    return 2 * npop_of(case) * (precision // 8) + (case.lattice - 1) * 4 + 4
 
 
 def moved_bytes_per_update(g, case, precision):
@@ -93,7 +107,7 @@ def moved_bytes_per_update(g, case, precision):
     a cell of a regular brick needs its 2*npop reals and 36 B of tile bases per 64 cells; any
     other cell the list row and the type byte on top, plus its entry of the irregular-cell list on levels that have bricks."""
     Q = case.lattice
-    npop = Q * (2 if case.ddf else 1) + (8 if case.collision == W.NUMEQ else 0)
+    npop = npop_of(case)
     s = precision // 8
     bricks = "bricks" in g.kernel_name()
     tot = upd = 0.0
@@ -121,6 +135,62 @@ def measured_peaks():
         except Exception:
             pass
     return {"hbm_gbs": FALLBACK_HBM_GBS}, "fallback (B200_PROFILING.md)"
+
+
+def kernel_source_hash():
+    """Hash of the kernel sources the committed ncu counters (profiles/traffic.csv) were taken with: a counter row whose
+    hash differs from the current sources is reported as stale instead of silently describing another kernel."""
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2504_04465_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:12]
+
+
+def committed_counters(key):
+    """Row `key` of profiles/traffic.csv (ncu counters of the dominant kernel, see profiles/traffic.md) or {}."""
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(tp):
+        return {}
+    try:
+        for r in csv.DictReader(open(tp)):
+            if r["key"] == key:
+                return {k: (v if k in ("key", "source", "kernel_hash") else float(v)) for k, v in r.items() if v not in ("", None)}
+    except Exception:
+        pass
+    return {}
+
+
+def roofline_blocks(case, precision, g, key, scale, upd_per_s, peak, peak_src, fma_peak):
+    """HBM roofline in the bytes this implementation must move (the list-addressed figure of SURVEY 8(d) beside it) and,
+    for the compute-heavy models, the ALU roofline against the FMA peak measured in this run."""
+    bpu = algorithmic_bytes_per_update(case, precision)
+    mbpu = moved_bytes_per_update(g, case, precision)
+    c = committed_counters(key)
+    stale = bool(c) and c.get("kernel_hash") != kernel_source_hash()
+    same_launch = bool(c) and scale == 1.0 and int(c.get("cells_per_launch", -1)) == int(g.n[0])
+    traffic = int(c["bytes_per_launch"]) if same_launch and "bytes_per_launch" in c and not stale else None
+    hbm = {"bound": "hbm", "achieved": upd_per_s * mbpu / 1e9, "peak": peak, "unit": "GB/s", "frac": upd_per_s * mbpu / 1e9 / peak,
+           "traffic": traffic, "traffic_source": c.get("source") if traffic else None,
+           "bytes_per_update": mbpu, "bytes_per_launch": int(g.n[0] * mbpu), "peak_source": peak_src,
+           "achieved_is": "bytes this implementation must move (brick cells: populations + 36 B per 64 cells; list cells: populations + list "
+                          "row + type byte) of all level sweeps of the timed region / its CUDA-event time (every launch is this kernel)",
+           "kernel": "%s, finest level (%d cells per launch)" % (g.kernel_name(), g.n[0]),
+           "list_addressed": {"bytes_per_update": bpu, "achieved": upd_per_s * bpu / 1e9, "frac": upd_per_s * bpu / 1e9 / peak,
+                              "what": "the same time charged with SURVEY 8(d)'s list-addressed algorithmic bytes (2 npop s + 4 (Q-1) + 4); "
+                                      "exceeds 1 where bricks remove the list traffic"},
+           "frac_of_nominal_8TBs": upd_per_s * mbpu / 1e9 / 8000.0}
+    hbm["frac_plausible"] = hbm["frac"] <= 1.05
+    alu = None
+    if fma_peak and "flop_per_update" in c:
+        tf = upd_per_s * c["flop_per_update"] / 1e12
+        alu = {"bound": "alu", "achieved": tf, "peak": fma_peak, "unit": "TFLOP/s", "frac": tf / fma_peak, "traffic": traffic,
+               "peak_source": "lbm_measure_fma_peak(%d) measured in this run" % precision,
+               "flop_per_update": c["flop_per_update"], "flop_source": c.get("source"),
+               "flop_is": "2 x FMA + ADD + MUL thread instructions of the finest level's launch / its cells (ncu smsp__sass_thread_inst_executed_op_*)",
+               "flop_counters_stale": stale or not same_launch, "pipe_pct_ncu": c.get("pipe_pct"),
+               "newton_steps_per_solve_at_capture": c.get("newton_steps_per_solve")}
+    return hbm, alu
 
 
 class ClockSampler:
@@ -159,6 +229,13 @@ class ClockSampler:
                     reasons.add(nme)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload_config(info, precision, n_levels, cells, cells_per_level, updates_per_step, world):
+    """The keys that name the workload: the same in the CUDA arm and in the reference arm."""
+    return dict(workload=info["workload"], precision=precision, cells=int(cells), levels=int(n_levels),
+                cells_per_level=[int(x) for x in cells_per_level], updates_per_step=int(updates_per_step),
+                step="one coarse step = %d fine steps" % (1 << (n_levels - 1)), parallelism="replicas x%d" % world)
 
 
 # ----------------------------------------------------------------------------- oracle legs (CPU)
@@ -208,10 +285,11 @@ def run_reference(args, case, info):
     if done < args.steps:
         sample += "; stopped at the %d s budget of the reference arm (%d steps asked)" % (REFERENCE_BUDGET_S, args.steps)
         args.steps = done
+    upd_coarse = sum(o.n[l] << (o.depth - l) for l in range(o.depth + 1))
     line = {"impl": "reference", "metric": "MLUPS (actual cell updates per second)", "value": v, "unit": "MLUPS", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": dict(workload=info["workload"], precision=64),
+            "config": workload_config(info, 64, o.depth + 1, o.ntot, o.n, upd_coarse, max(args.gpus, 1)),
             "cpu_baseline": {"value": v, "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -235,27 +313,82 @@ def aggregate_mlups(updates_per_rank_step, steps, world, ms):
     return updates_per_rank_step * steps * world / (ms * 1e-3) / 1e6
 
 
-def also_measure(lbm, name, precision, dev, peak):
-    """Device-resident throughput of another workload with its default step count, for the `also` entries of the default
+_FMA_PEAK = {}
+
+
+def fma_peak_of(lbm, precision):
+    """FMA peak of the plain fp64 / fp32 pipe, measured once per run (1 s) -- denominator of the ALU rooflines."""
+    if precision not in _FMA_PEAK:
+        _FMA_PEAK[precision] = lbm.measure_fma_peak(precision, 1.0)[0]
+    return _FMA_PEAK[precision]
+
+
+def wants_alu(case):
+    return case.collision == W.NUMEQ or (case.lattice == 37 and case.ddf)
+
+
+def newton_block(g, it0, ns0, updates):
+    it1, ns1 = g.newton_iterations()
+    if ns1 == ns0:
+        return None
+    return {"steps_per_solve": (it1 - it0) / (ns1 - ns0), "solves_per_update": (ns1 - ns0) / max(updates, 1),
+            "what": "Newton steps (unconditional polish step included) per equilibrium solve in the timed region, counted by the kernels "
+                    "(lbm_newton_iterations); the paper: about one iteration on smooth fields with a warm start (P:124)"}
+
+
+def parse_also(entry, precision):
+    parts = entry.split("@")
+    opts = dict(precision=precision, addressing="auto")
+    for o in parts[1:]:
+        if o in ("f32", "f64"):
+            opts["precision"] = int(o[1:])
+        elif o in ADDRESSING:
+            opts["addressing"] = o
+        else:
+            raise SystemExit("unknown option %r in --also entry %r" % (o, entry))
+    return parts[0], opts
+
+
+def also_measure(lbm, entry, precision, dev, peak, peak_src):
+    """Device-resident throughput of another workload with its own step count, for the `also` entries of the default
     line (same timing rules: 3 warm-up steps, CUDA events on the bound stream around the replayed graphs)."""
+    name, opts = parse_also(entry, precision)
+    prec = opts["precision"]
     case, info = make_case(name, 1.0)
-    g = lbm.Grid.from_case(case, precision=precision)
+    steps = info.get("also_steps", info["steps"])
+    t0 = time.perf_counter()
+    g = lbm.Grid.from_case(case, precision=prec, addressing=ADDRESSING[opts["addressing"]])
     g.bind(dev)
     cells = [g.cells(l)[:2] for l in range(g.depth + 1)]
     rc = g.init_fields(*W.eval_fields(case, cells))
     assert rc == 0, rc
+    t_build = time.perf_counter() - t0
     g.step(3)
     assert g.sync() == 0
-    g.step(info["steps"])
+    it0, ns0 = g.newton_iterations()
+    g.step(steps)
     ms = g.last_step_ms()
-    assert g.sync() == 0
+    status = g.sync()
+    assert status == 0, "device status %d after the timed region of %s" % (status, entry)
     upd = int(g.info.updates_per_coarse_step)
-    bpu = algorithmic_bytes_per_update(case, precision)
-    v = upd * info["steps"] / (ms * 1e-3) / 1e6
-    out = {"workload": info["workload"], "dtype": "f%d" % precision, "value": v, "unit": "MLUPS", "steps": info["steps"],
-           "ms_per_step": ms / info["steps"], "cells": g.ntot, "gpu_launches": int(g.info.launches_per_coarse_step) * info["steps"],
-           "roofline_frac": v * 1e6 * bpu / 1e9 / peak, "roofline_frac_moved": v * 1e6 * moved_bytes_per_update(g, case, precision) / 1e9 / peak,
-           "kernel": g.kernel_name()}
+    v = upd * steps / (ms * 1e-3) / 1e6
+    key = "%s_f%d" % (name, prec) + ("" if opts["addressing"] == "auto" else "@" + opts["addressing"])
+    hbm, alu = roofline_blocks(case, prec, g, key, 1.0, v * 1e6, peak, peak_src, fma_peak_of(lbm, prec) if wants_alu(case) else None)
+    out = {"workload": info["workload"], "entry": entry, "dtype": "f%d" % prec, "value": v, "unit": "MLUPS", "steps": steps,
+           "ms_per_step": ms / steps, "cells": g.ntot, "levels": g.depth + 1, "gpu_launches": int(g.info.launches_per_coarse_step) * steps,
+           "kernel": g.kernel_name(), "build_s": t_build, "arena_bytes": int(g.info.arena_bytes),
+           "mlups_paper_eq13": g.ntot * (1 << g.depth) * steps / (ms * 1e-3) / 1e6}
+    if case.collision == W.NUMEQ and alu is not None:
+        out["roofline"], out["roofline_hbm"] = alu, hbm
+    else:
+        out["roofline"] = hbm
+        if alu is not None:
+            out["roofline_alu"] = alu
+    nb = newton_block(g, it0, ns0, upd * steps)
+    if nb:
+        out["newton"] = nb
+    if info.get("paper_mlups") and prec == 32:
+        out["vs_paper_table3a_a100"] = out["mlups_paper_eq13"] / info["paper_mlups"]
     g.close()
     return out
 
@@ -268,12 +401,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="cylinder")
     ap.add_argument("--precision", type=int, default=64, choices=[32, 64])
+    ap.add_argument("--addressing", default="auto", choices=sorted(ADDRESSING), help="lbm_config.addressing: auto = regular bricks on "
+                    "large levels, list = the list-addressed kernel on every level, bricks = bricks on every level")
     ap.add_argument("--scale", type=float, default=1.0, help="linear scale of the workload (1 = BASELINE size)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0, help="0 disables the cpu_baseline leg")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--also", default=None, help="comma list of other workloads measured briefly into the line's `also` "
-                    "(default for the default workload: cavity = configs[1] and uniform = configs[0] scaled; 'none' disables)")
+                    "(default for the default workload: %s; 'none' disables)" % DEFAULT_ALSO)
     args = ap.parse_args()
     case, info = make_case(args.workload, args.scale)
     if args.steps is None:
@@ -301,7 +436,7 @@ def main():
         torch.cuda.synchronize()
 
     t_build = time.perf_counter()
-    g = lbm.Grid.from_case(case, precision=args.precision)
+    g = lbm.Grid.from_case(case, precision=args.precision, addressing=ADDRESSING[args.addressing])
     g.bind(dev)
     ntot = g.ntot
     pin = lambda: torch.empty(ntot, dtype=torch.float64).pin_memory().numpy()
@@ -320,13 +455,14 @@ def main():
     g.step(args.warmup)
     assert g.sync() == 0
     # burst figure (GPU still cool, ~30 ms region: comparable with MEASURED_PEAKS' best-of-10 copy); the headline
-    # `value` below is the sustained figure over the full K steps, which on these 1 kW parts runs under sw_power_cap
+    # `value` below is the figure over the full K steps, which for long regions on these 1 kW parts runs under sw_power_cap
     g.step(3)
     est = max(g.last_step_ms() / 3, 1e-4)
     kb = int(min(max(3, 30.0 / est), max(3, args.steps)))
     g.step(kb)
     burst_ms = g.last_step_ms() / kb
     assert g.sync() == 0
+    it0, ns0 = g.newton_iterations()
     barrier()
     clk = ClockSampler(local)
     t0 = time.perf_counter()
@@ -337,6 +473,7 @@ def main():
     wall = time.perf_counter() - t0
     clocks = clk.stop()
     assert status == 0, "device status %d after the timed region" % status
+    newton = newton_block(g, it0, ns0, upd * args.steps)
 
     # ---- end to end through the C ABI with pinned host buffers, every step: H2D fields -> step -> D2H macroscopic
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -363,35 +500,12 @@ def main():
 
     K = args.steps
     mlups = aggregate_mlups(upd, K, world, ms)
-    bpu = algorithmic_bytes_per_update(case, args.precision)
-    mbpu = moved_bytes_per_update(g, case, args.precision)
     peaks, peak_src = measured_peaks()
     peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
-    achieved = upd * K * bpu / (ms * 1e-3) / 1e9          # this rank's kernel: all launches of the region are the sweep kernel
-    # counters of the dominant kernel (finest level's sweep) from the committed ncu --set full captures
-    traffic = traffic_src = None
-    counters = {}
-    tp = os.path.join(ROOT, "profiles", "traffic.csv")
-    if os.path.exists(tp):
-        try:
-            import csv
-            rows = {r["key"]: r for r in csv.DictReader(open(tp))}
-            r = rows.get("%s_f%d" % (args.workload, args.precision))
-            if r:
-                counters = {k: (float(v) if k not in ("key", "source") else v) for k, v in r.items() if v != ""}
-            if args.scale == 1.0 and int(counters.get("cells_per_launch", -1)) == int(g.n[0]):
-                traffic, traffic_src = int(counters["bytes_per_launch"]), counters["source"]
-        except Exception:
-            counters = {}
-    # ALU-bound path (numerical equilibria): fp64 flop per update from the ncu capture against the FMA peak measured now
-    alu = None
-    if case.collision == W.NUMEQ and "fp64_flop_per_update" in counters and args.precision == 64:
-        fma_peak, _ = lbm.measure_fma_peak(64, 1.0)
-        tf = upd * K * counters["fp64_flop_per_update"] / (ms * 1e-3) / 1e12
-        alu = {"bound": "alu", "achieved": tf, "peak": fma_peak, "unit": "TFLOP/s", "frac": tf / fma_peak, "traffic": traffic,
-               "peak_source": "lbm_measure_fma_peak(64) measured in this run (148 SMs x 64 fp64 FMA lanes x clock)",
-               "flop_per_update": counters["fp64_flop_per_update"], "flop_source": "profiles/traffic.md",
-               "fp64_pipe_pct_ncu": counters.get("fp64_pipe_pct")}
+    key = "%s_f%d" % (args.workload, args.precision) + ("" if args.addressing == "auto" else "@" + args.addressing)
+    rank_upd_per_s = upd * K / (ms * 1e-3)               # this rank's kernel: every launch of the region is the sweep kernel
+    hbm, alu = roofline_blocks(case, args.precision, g, key, args.scale, rank_upd_per_s, peak, peak_src,
+                               fma_peak_of(lbm, args.precision) if wants_alu(case) else None)
     n_all = ntot
     depth = g.depth
     # vs_baseline only where BASELINE.md holds the paper's number for this exact metric and workload: Table 3a, Eq. 13
@@ -399,30 +513,22 @@ def main():
     vs_baseline = None
     if info.get("paper_mlups") and args.precision == 32 and args.scale == 1.0 and world == 1:
         vs_baseline = n_all * (1 << depth) * K / (ms * 1e-3) / 1e6 / info["paper_mlups"]
+    config = workload_config(info, args.precision, depth + 1, n_all, g.n, upd, world)
+    config["l2"] = ("inputs larger than L2 (state %.0f MB)" % (g.info.arena_bytes / 1e6) if g.info.arena_bytes > 4 * 126e6
+                    else "working set %.0f MB fits L2: launch-latency-bound case, no flush" % (g.info.arena_bytes / 1e6))
     line = {
         "metric": "MLUPS (actual cell updates per second)", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K,
         "warmup": args.warmup, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": vs_baseline,
-        "dtype": "f%d" % args.precision, "data": "synthetic",
-        "config": dict(workload=info["workload"], precision=args.precision, cells=n_all, levels=depth + 1,
-                       cells_per_level=g.n, updates_per_step=upd, step="one coarse step = %d fine steps" % (1 << depth),
-                       parallelism="replicas x%d" % world, l2="inputs larger than L2 (state %.0f MB)" % (g.info.arena_bytes / 1e6)
-                       if g.info.arena_bytes > 4 * 126e6 else "working set %.0f MB fits L2: launch-latency-bound case, no flush" % (g.info.arena_bytes / 1e6),
-                       kernel=g.kernel_name(), brick_cell_share=[round(64 * int(g.info.n_bricks[l]) / max(g.n[l], 1), 4) if g.n[l] >= int(g.info.brick_min_level_cells) else 0.0
-                                         for l in range(depth + 1)]),
+        "dtype": "f%d" % args.precision, "data": "synthetic", "config": config,
+        "kernel": {"name": g.kernel_name(), "addressing": args.addressing, "arena_bytes": int(g.info.arena_bytes),
+                   "brick_cell_share": [round(64 * int(g.info.n_bricks[l]) / max(g.n[l], 1), 4) if g.n[l] >= int(g.info.brick_min_level_cells) else 0.0
+                                        for l in range(depth + 1)]},
         "mlups": {"actual": mlups, "paper_eq13": n_all * (1 << depth) * K * world / (ms * 1e-3) / 1e6,
                   "fine_equivalent": fine_equivalent_cells(case) * (1 << depth) * K * world / (ms * 1e-3) / 1e6},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "traffic_source": traffic_src,
-                     "algorithmic_bytes_per_launch": int(g.n[0]) * bpu, "kernel": "%s, finest level (%d cells per launch)" % (g.kernel_name(), g.n[0]),
-                     "achieved_is": "algorithmic bytes of all level sweeps of the timed region / its CUDA-event time (every launch is this kernel)",
-                     "peak_source": peak_src, "bytes_per_update": bpu,
-                     "moved_bytes_per_update": mbpu, "moved": achieved * mbpu / bpu, "frac_moved": achieved * mbpu / bpu / peak,
-                     "note": "achieved/frac use the list-addressed method's algorithmic bytes (SURVEY 8(d)); with regular bricks the kernel "
-                             "moves fewer bytes than that, so frac can exceed 1: moved/frac_moved count what this implementation must move",
-                     "frac_of_nominal_8TBs": achieved / 8000.0},
+        "roofline": hbm,
         "burst": {"steps": kb, "ms_per_step": burst_ms, "value": upd / (burst_ms * 1e-3) / 1e6, "unit": "MLUPS (this rank)",
-                  "roofline_frac": upd * bpu / (burst_ms * 1e-3) / 1e9 / peak,
-                  "what": "short region right after warm-up, before the power cap settles; `value` is the sustained figure"},
+                  "roofline_frac": upd * hbm["bytes_per_update"] / (burst_ms * 1e-3) / 1e9 / peak,
+                  "what": "short region right after warm-up, before the power cap settles"},
         "e2e": {"value": upd * world / (e2e_ms * 1e-3) / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 4 * 8 * ntot,
                 "d2h_bytes_per_step": 4 * 8 * ntot, "ms_per_step": e2e_ms,
                 "what": "lbm_init_fields (pinned host rho,u,T) + lbm_step(1) + lbm_get_macroscopic (pinned host), every step"},
@@ -430,16 +536,20 @@ def main():
         "clocks": clocks,
         "wall_s_timed_region": wall, "build_s": t_build,
     }
-    if alu is not None:       # the HBM view stays beside it
-        line["roofline_hbm"] = line["roofline"]
-        line["roofline"] = alu
-    elif "fp64_pipe_pct" in counters:
-        line["roofline"]["fp64_pipe_pct_ncu"] = counters["fp64_pipe_pct"]
-        line["roofline"]["fp64_tflops"] = upd * K * counters["fp64_flop_per_update"] / (ms * 1e-3) / 1e12
-    also = args.also if args.also is not None else ("cavity,uniform" if args.workload == "cylinder" and args.scale == 1.0 else "none")
+    if case.collision == W.NUMEQ and alu is not None:       # ALU-bound path: the HBM view stays beside it
+        line["roofline"], line["roofline_hbm"] = alu, hbm
+    elif alu is not None:
+        line["roofline_alu"] = alu
+    if newton:
+        line["newton"] = newton
+    also = args.also if args.also is not None else (DEFAULT_ALSO if args.workload == "cylinder" and args.scale == 1.0 and args.addressing == "auto" else "none")
     if also != "none" and world == 1:
         g.close()                # release the arena before building the next grid
-        line["also"] = [also_measure(lbm, w, args.precision, dev, peak) for w in also.split(",") if w]
+        del h_in, h_out
+        line["also"] = []
+        for entry in [w for w in also.split(",") if w]:
+            line["also"].append(also_measure(lbm, entry, args.precision, dev, peak, peak_src))
+            torch.cuda.empty_cache()
     if args.cpu_baseline_seconds > 0 and world >= 1:
         o = oracle_grid(case)
         v, nf, nu, dt = oracle_rate(o, args.cpu_baseline_seconds)

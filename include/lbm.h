@@ -49,6 +49,8 @@ enum { LBM_BC_PERIODIC = 0, LBM_BC_WALL = 1, LBM_BC_MOVING_WALL = 2, LBM_BC_INFL
 enum { LBM_FLUID = 0, LBM_FINE_GHOST = 1, LBM_COARSE_GHOST = 2, LBM_NEUMANN = 3, LBM_DIRICHLET = 4 };
 /* negative link values in the neighbour list */
 enum { LBM_LINK_NONE = -1, LBM_LINK_WALL = -2, LBM_LINK_VBB0 = -3 /* -3-side */ };
+/* device addressing modes (lbm_config.addressing) */
+enum { LBM_ADDR_AUTO = 0, LBM_ADDR_LIST = 1, LBM_ADDR_BRICKS = 2 };
 /* error codes */
 enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_EMESH = -3, LBM_ECUDA = -4,
        LBM_EUNSTABLE = -5 /* non-finite or non-positive density */,
@@ -78,6 +80,13 @@ typedef struct {
    * (x0, y0) in finest-level units; before each collision rho is relaxed to rho (1 - sigma) + sigma rho_inf at unchanged
    * velocity and non-equilibrium part.  sigma_max = 0: off.  Weakly compressible models only (LBM_EINVAL otherwise). */
   double sponge_x0, sponge_y0, sponge_r0, sponge_r1, sponge_sigma_max, sponge_rho_inf;
+  /* Device-path options (they change how the kernels address memory and how launches are chained, never the result):
+   * addressing: LBM_ADDR_AUTO = regular 8x8 bricks by tile arithmetic on levels of >= 2^18 stored cells and the neighbour
+   * list elsewhere; LBM_ADDR_LIST = the list-addressed kernel of north_star on every level;
+   * LBM_ADDR_BRICKS = bricks on every level that has some.  no_pdl = 1: plain stream order between level sweeps instead
+   * of programmatic dependent launch edges. */
+  int addressing;
+  int no_pdl;
 } lbm_config;
 
 typedef struct {
@@ -113,6 +122,11 @@ void lbm_destroy(lbm_grid* g);
 
 int lbm_grid_query(const lbm_grid* g, lbm_grid_info* out);
 
+/* Enumerates the model combinations this build has kernels for: fills lattice, precision, collision, ddf, sensor of *out
+ * (everything else zero) for index = 0, 1, ... and returns LBM_EINVAL past the last one.  Any other combination makes
+ * lbm_grid_create return LBM_EUNSUPPORTED.  HOST out.  No CUDA call. */
+int lbm_supported_model(int index, lbm_config* out);
+
 /* Bit-exact tables (HOST outputs, caller-owned, any may be NULL):
  *  cells:    ix, iy, type, aux per stored cell (aux: ghost-list index of a coarse ghost, source cell of a
  *            Neumann / Dirichlet cell, -1 otherwise)
@@ -137,9 +151,11 @@ int lbm_get_sponge(const lbm_grid* g, int level, double* sigma);
  * tiles9: HOST out, 9*n_bricks[level] int32; table: HOST out, (Q-1)*64 uint16; either may be NULL. */
 int lbm_get_bricks(const lbm_grid* g, int level, int32_t* tiles9, uint16_t* table);
 
-/* Attaches caller-owned DEVICE memory (>= arena_bytes, 256-byte aligned) and a CUDA stream
- * (cudaStream_t passed as void*; NULL = legacy default stream), uploads the mesh tables and captures
- * the CUDA graphs of one coarse step.  The arena must stay valid until lbm_destroy. */
+/* Attaches caller-owned DEVICE memory (>= arena_bytes, 256-byte aligned, on the CURRENT device of the calling thread)
+ * and a CUDA stream of that device (cudaStream_t passed as void*; NULL = the library creates and owns a non-blocking
+ * stream) and uploads the mesh tables.  The device is remembered: every later call on this grid selects it for its own
+ * duration and restores the caller's current device before returning.  The CUDA graphs of the coarse step are captured on
+ * first use by lbm_step.  The arena must stay valid until lbm_destroy.  On failure nothing stays attached. */
 int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream);
 
 /* Sets every stored cell (ghosts included) to the equilibrium of the given macroscopic fields at its own
@@ -182,8 +198,13 @@ int lbm_set_populations(lbm_grid* g, int level, int which, const double* in);
 /* Device-time of the work enqueued by the last lbm_step call, in milliseconds (CUDA events recorded on
  * the bound stream around it); synchronises.  Negative error code on failure. */
 double lbm_last_step_ms(lbm_grid* g);
+/* Newton statistics of the numerical-equilibrium models ("converges in just one iteration on average"):
+ * Newton steps taken (the unconditional polish step of reading S14 included) and equilibrium solves performed on the device
+ * since lbm_grid_bind (initialisation, iteration-0 coupling, every colliding or Dirichlet cell of every sweep), counted by
+ * the kernels themselves.  HOST outputs, either may be NULL; zeros for polynomial models.  Synchronises. */
+int lbm_newton_iterations(lbm_grid* g, int64_t* iterations, int64_t* solves);
 /* Name of the compiled sweep kernel this grid dispatches to (static string), for profiles; says whether the
- * compressed addressing of regular bricks is in use (environment LBM_NO_BRICKS=1 at bind time turns it off). */
+ * compressed addressing of regular bricks is in use (lbm_config.addressing). */
 const char* lbm_kernel_name(const lbm_grid* g);
 
 

@@ -68,11 +68,12 @@ struct lbm_grid {
   int64_t n_total = 0, launches_per_coarse = 0, updates_per_coarse = 0;
   size_t arena_bytes = 0, off_status = 0, off_scratch = 0, scratch_doubles = 0;
   bool bound = false, inited = false, own_stream = false;
-  int64_t brick_min_cells = BRICK_MIN_LEVEL_CELLS;   // levels below this go through the list (LBM_BRICK_MIN_CELLS overrides)
-  bool bricks = false;                            // compressed addressing of regular bricks (LBM_NO_BRICKS=1 disables)
+  int64_t brick_min_cells = BRICK_MIN_LEVEL_CELLS;   // levels below this go through the list (lbm_config.addressing: AUTO)
+  bool bricks = false;                            // compressed addressing of regular bricks (off for LBM_ADDR_LIST)
+  int device = -1;                                // device of the arena, selected by every entry point for its own duration
   size_t off_tab = 0;
   unsigned short* d_tab = nullptr;
-  bool pdl = true;                                // programmatic dependent launch between level sweeps (LBM_NO_PDL=1 disables)
+  bool pdl = true;                                // programmatic dependent launch between level sweeps (lbm_config.no_pdl)
   char* arena = nullptr;
   cudaStream_t stream = nullptr;
   int* d_status = nullptr;
@@ -86,6 +87,19 @@ struct lbm_grid {
 };
 
 namespace {
+
+// Selects the grid's device for the duration of one ABI call and restores the caller's current device afterwards (the
+// library links the CUDA runtime statically: the "current device" it sees is the calling thread's).
+struct DeviceScope {
+  int prev = -1;
+  bool changed = false;
+  explicit DeviceScope(int dev) {
+    if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) changed = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceScope() { if (changed) cudaSetDevice(prev); }
+  DeviceScope(const DeviceScope&) = delete;
+  DeviceScope& operator=(const DeviceScope&) = delete;
+};
 
 #define CK(call)                                  \
   do {                                            \
@@ -167,7 +181,7 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   } else {
     rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream, g->ks->cells_per_thread, g->pdl);
   }
-  cur[l] ^= 1;
+  if (rc == LBM_OK) cur[l] ^= 1;
   return rc;
 }
 
@@ -208,6 +222,8 @@ int status_code(lbm_grid* g) {
   return LBM_OK;
 }
 
+void release_device_objects(lbm_grid* g);
+
 int pop_range(const lbm_grid* g, int which, int* off, int* cnt) {
   const bool ddf = g->hg.cfg.ddf != 0, numeq = g->hg.cfg.collision == LBM_NUMEQ;
   if (which == 0) { *off = 0; *cnt = g->Q; return LBM_OK; }
@@ -228,6 +244,7 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
   if (cfg->collision < LBM_BGK || cfg->collision > LBM_NUMEQ) return LBM_EINVAL;
   if (cfg->collision == LBM_RR && cfg->ddf) return LBM_EINVAL;     // RR is defined for the athermal models only
   if (!(cfg->tau0 >= 0.5)) return LBM_EINVAL;
+  if (cfg->addressing < LBM_ADDR_AUTO || cfg->addressing > LBM_ADDR_BRICKS) return LBM_EINVAL;
   // the sponge relaxes rho = p / T0: weakly compressible models only
   if (cfg->sponge_sigma_max != 0.0 && (cfg->ddf || cfg->collision == LBM_NUMEQ || !(cfg->sponge_sigma_max > 0.0) ||
                                        !(cfg->sponge_sigma_max <= 1.0) || !(cfg->sponge_r1 > cfg->sponge_r0) || !(cfg->sponge_r0 >= 0.0)))
@@ -250,6 +267,9 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
     g->depth = cfg->depth;
     g->esize = cfg->precision / 8;
     g->npop = lat.Q * (cfg->ddf ? 2 : 1) + (cfg->collision == LBM_NUMEQ ? LBM_NLAMBDA : 0);
+    g->bricks = ks->sweep_bricks != nullptr && cfg->addressing != LBM_ADDR_LIST;
+    g->brick_min_cells = !g->bricks ? INT64_MAX : cfg->addressing == LBM_ADDR_BRICKS ? 0 : BRICK_MIN_LEVEL_CELLS;
+    g->pdl = cfg->no_pdl == 0;
     ModelParams& mp = g->mp;
     mp.gamma = cfg->gamma; mp.sensor_A = cfg->sensor_A; mp.T0 = cfg->T0; mp.newton_tol = cfg->newton_tol;
     mp.newton_max_iter = cfg->newton_max_iter; mp.trace_eq = cfg->trace_eq;
@@ -298,14 +318,9 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
 void lbm_destroy(lbm_grid* g) {
   if (!g) return;
   if (g->bound) {
+    DeviceScope dev(g->device);
     cudaStreamSynchronize(g->stream);
-    for (int p = 0; p < 2; ++p) {
-      if (g->g1[p]) cudaGraphExecDestroy(g->g1[p]);
-      if (g->gk[p]) cudaGraphExecDestroy(g->gk[p]);
-    }
-    if (g->ev0) cudaEventDestroy(g->ev0);
-    if (g->ev1) cudaEventDestroy(g->ev1);
-    if (g->own_stream) cudaStreamDestroy(g->stream);
+    release_device_objects(g);
   }
   delete g;
 }
@@ -388,12 +403,22 @@ int lbm_get_schedule(const lbm_grid* g, int32_t* k_of, int32_t* level_of, int ca
   return n;
 }
 
-int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream) {
-  if (!g || !dev_arena) return LBM_EINVAL;
-  if (g->bound) return LBM_ESTATE;
-  if (nbytes < g->arena_bytes || ((uintptr_t)dev_arena % ALIGN) != 0) return LBM_EINVAL;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LBM_ECUDA;   // no CPU fallback
+}  // extern "C"
+
+namespace {
+
+void release_device_objects(lbm_grid* g) {
+  for (int p = 0; p < 2; ++p) {
+    if (g->g1[p]) { cudaGraphExecDestroy(g->g1[p]); g->g1[p] = nullptr; }
+    if (g->gk[p]) { cudaGraphExecDestroy(g->gk[p]); g->gk[p] = nullptr; }
+  }
+  if (g->ev0) { cudaEventDestroy(g->ev0); g->ev0 = nullptr; }
+  if (g->ev1) { cudaEventDestroy(g->ev1); g->ev1 = nullptr; }
+  if (g->own_stream && g->stream) cudaStreamDestroy(g->stream);
+  g->stream = nullptr; g->own_stream = false;
+}
+
+int bind_impl(lbm_grid* g, void* dev_arena, void* cuda_stream) {
   g->arena = (char*)dev_arena;
   if (cuda_stream) {
     g->stream = (cudaStream_t)cuda_stream;
@@ -442,11 +467,6 @@ int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream
   CK(cudaStreamSynchronize(g->stream));
   CK(cudaEventCreate(&g->ev0));
   CK(cudaEventCreate(&g->ev1));
-  g->bound = true;
-  if (const char* e = getenv("LBM_NO_PDL")) g->pdl = !(e[0] == '1');
-  g->bricks = g->ks->sweep_bricks != nullptr;
-  if (const char* e = getenv("LBM_NO_BRICKS")) g->bricks = g->bricks && !(e[0] == '1');
-  if (const char* e = getenv("LBM_BRICK_MIN_CELLS")) g->brick_min_cells = atoll(e);
   // graphs (one coarse step from either parity of the coarsest level; K steps for launch-bound grids) are captured on
   // first use by lbm_step and dropped when a parameter baked into their kernel arguments changes
   g->K = 0;
@@ -458,9 +478,36 @@ int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream
   return LBM_OK;
 }
 
+}  // namespace
+
+extern "C" {
+
+int lbm_grid_bind(lbm_grid* g, void* dev_arena, size_t nbytes, void* cuda_stream) {
+  if (!g || !dev_arena) return LBM_EINVAL;
+  if (g->bound) return LBM_ESTATE;
+  if (nbytes < g->arena_bytes || ((uintptr_t)dev_arena % ALIGN) != 0) return LBM_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return LBM_ECUDA;   // no CPU fallback
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, dev_arena) != cudaSuccess) { cudaGetLastError(); return LBM_ECUDA; }
+  if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) return LBM_EINVAL;   // host pointers are not an arena
+  g->device = at.device;
+  DeviceScope dev(g->device);
+  const int rc = bind_impl(g, dev_arena, cuda_stream);
+  if (rc != LBM_OK) {            // nothing stays attached: the stream and events created so far are released
+    release_device_objects(g);
+    g->arena = nullptr; g->device = -1;
+    return rc;
+  }
+  g->bound = true;
+  return LBM_OK;
+}
+
 int lbm_init_fields(lbm_grid* g, const double* rho, const double* ux, const double* uy, const double* T) {
   if (!g || !rho || !ux || !uy) return LBM_EINVAL;
   if (!g->bound) return LBM_ESTATE;
+  DeviceScope dev(g->device);
+  g->inited = false;
   const size_t N = (size_t)g->n_total;
   double* d_rho = g->d_scratch;
   double* d_ux = d_rho + N;
@@ -502,9 +549,14 @@ int lbm_init_fields(lbm_grid* g, const double* rho, const double* ux, const doub
 int lbm_step_fine(lbm_grid* g, int n) {
   if (!g || n < 0) return LBM_EINVAL;
   if (!g->bound || !g->inited) return LBM_ESTATE;
+  DeviceScope dev(g->device);
   const int d = g->depth;
   std::vector<int> cur((size_t)d + 1);
   for (int l = 0; l <= d; ++l) cur[l] = g->dl[l].cur;
+  // a launch that fails in the middle of a fine step leaves some levels advanced and others not: the grid is then marked
+  // uninitialised (every compute call returns LBM_ESTATE until the next lbm_init_fields) instead of running on with
+  // buffer parities that no longer describe the device state
+  g->inited = false;
   CK(cudaEventRecord(g->ev0, g->stream));
   for (int s = 0; s < n; ++s) {
     const int64_t k = g->kfine + 1;               // schedule of DESIGN.md Sec. 6 rule 9 at fine step k
@@ -514,9 +566,10 @@ int lbm_step_fine(lbm_grid* g, int n) {
       if (rc) return rc;
     }
     g->kfine = k % ((int64_t)1 << d);
+    for (int l = 0; l <= d; ++l) g->dl[l].cur = cur[l];
   }
   CK(cudaEventRecord(g->ev1, g->stream));
-  for (int l = 0; l <= d; ++l) g->dl[l].cur = cur[l];
+  g->inited = true;
   g->timed = true;
   return LBM_OK;
 }
@@ -525,6 +578,7 @@ int lbm_step(lbm_grid* g, int n) {
   if (!g || n < 0) return LBM_EINVAL;
   if (!g->bound || !g->inited) return LBM_ESTATE;
   if (g->kfine != 0) return LBM_ESTATE;           // graphs start at a coarse-step boundary
+  DeviceScope dev(g->device);
   int& p = g->dl[g->depth].cur;
   // capture what this call needs before the timed region starts: n = nk launches of the K-step graph (parity kept) and
   // r single steps that alternate the parity
@@ -532,6 +586,7 @@ int lbm_step(lbm_grid* g, int n) {
   if (nk > 0 && !g->gk[p]) { int rc = capture(g, p, g->K, &g->gk[p]); if (rc) return rc; }
   if (r >= 1 && !g->g1[p]) { int rc = capture(g, p, 1, &g->g1[p]); if (rc) return rc; }
   if (r >= 2 && !g->g1[p ^ 1]) { int rc = capture(g, p ^ 1, 1, &g->g1[p ^ 1]); if (rc) return rc; }
+  g->inited = false;                                // see lbm_step_fine: restored once everything is enqueued
   CK(cudaEventRecord(g->ev0, g->stream));
   while (n > 0) {
     if (g->K >= 2 && n >= g->K) {
@@ -539,11 +594,12 @@ int lbm_step(lbm_grid* g, int n) {
       n -= g->K;
     } else {
       CK(cudaGraphLaunch(g->g1[p], g->stream));
-      p ^= 1;
+      p ^= 1;                                       // one coarse step flips the coarsest level once, every other level an even number of times
       n -= 1;
     }
   }
   CK(cudaEventRecord(g->ev1, g->stream));
+  g->inited = true;
   g->timed = true;
   return LBM_OK;
 }
@@ -551,6 +607,7 @@ int lbm_step(lbm_grid* g, int n) {
 namespace {
 void drop_graphs(lbm_grid* g) {
   if (!g->bound) return;
+  DeviceScope dev(g->device);
   cudaStreamSynchronize(g->stream);
   for (int p = 0; p < 2; ++p) {
     if (g->g1[p]) { cudaGraphExecDestroy(g->g1[p]); g->g1[p] = nullptr; }
@@ -578,26 +635,58 @@ int lbm_set_boundary_state(lbm_grid* g, int side, double rho, double ux, double 
 int lbm_sync(lbm_grid* g) {
   if (!g) return LBM_EINVAL;
   if (!g->bound) return LBM_ESTATE;
+  DeviceScope dev(g->device);
   return status_code(g);
 }
 
 double lbm_last_step_ms(lbm_grid* g) {
   if (!g) return (double)LBM_EINVAL;
   if (!g->bound || !g->timed) return (double)LBM_ESTATE;
+  DeviceScope dev(g->device);
   if (cudaEventSynchronize(g->ev1) != cudaSuccess) return (double)LBM_ECUDA;
   float ms = 0.f;
   if (cudaEventElapsedTime(&ms, g->ev0, g->ev1) != cudaSuccess) return (double)LBM_ECUDA;
   return (double)ms;
 }
 
+int lbm_supported_model(int index, lbm_config* out) {
+  if (index < 0 || !out) return LBM_EINVAL;
+  const KernelSet* sets = nullptr;
+  int base = 0;
+  for (int lat = 0; lat < 4; ++lat) {
+    const int n = lat == 0 ? kernel_sets_q9(&sets) : lat == 1 ? kernel_sets_q13(&sets) : lat == 2 ? kernel_sets_q21(&sets) : kernel_sets_q37(&sets);
+    if (index < base + n) {
+      const KernelSet& k = sets[index - base];
+      memset(out, 0, sizeof(*out));
+      out->lattice = k.Q; out->precision = k.precision; out->collision = k.collision; out->ddf = k.ddf; out->sensor = k.sensor;
+      return LBM_OK;
+    }
+    base += n;
+  }
+  return LBM_EINVAL;
+}
+
+int lbm_newton_iterations(lbm_grid* g, int64_t* iterations, int64_t* solves) {
+  if (!g) return LBM_EINVAL;
+  if (!g->bound) return LBM_ESTATE;
+  DeviceScope dev(g->device);
+  unsigned long long h[2] = {0ull, 0ull};
+  CK(cudaMemcpyAsync(h, (const char*)g->d_status + NEWTON_COUNTER_OFFSET, sizeof(h), cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  if (iterations) *iterations = (int64_t)h[0];
+  if (solves) *solves = (int64_t)h[1];
+  return LBM_OK;
+}
+
 const char* lbm_kernel_name(const lbm_grid* g) {
   if (!g) return "";
-  return (g->bound ? g->bricks : g->ks->sweep_bricks != nullptr) ? g->ks->bricks_name : g->ks->name;
+  return g->bricks ? g->ks->bricks_name : g->ks->name;
 }
 
 int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double* T) {
   if (!g) return LBM_EINVAL;
   if (!g->bound || !g->inited) return LBM_ESTATE;
+  DeviceScope dev(g->device);
   const size_t N = (size_t)g->n_total;
   double* d[4] = {g->d_scratch, g->d_scratch + N, g->d_scratch + 2 * N, g->d_scratch + 3 * N};
   int64_t base = 0;
@@ -621,6 +710,7 @@ int lbm_get_macroscopic_at(lbm_grid* g, int l, int n, const int32_t* cells, doub
   if (!g || !cells || n < 0 || l < 0 || l > g->depth) return LBM_EINVAL;
   if (!g->bound || !g->inited) return LBM_ESTATE;
   if (n == 0) return LBM_OK;
+  DeviceScope dev(g->device);
   DevLevel& L = g->dl[l];
   if ((size_t)n * 5 + 8 > g->scratch_doubles) return LBM_EINVAL;
   for (int k = 0; k < n; ++k)
@@ -645,6 +735,7 @@ int lbm_get_populations(lbm_grid* g, int l, int which, double* out) {
   if (!g->bound) return LBM_ESTATE;
   int off, cnt;
   if (pop_range(g, which, &off, &cnt)) return LBM_EINVAL;
+  DeviceScope dev(g->device);
   DevLevel& L = g->dl[l];
   if (L.n == 0) return LBM_OK;
   const long long tot = (long long)L.n * cnt;
@@ -664,6 +755,7 @@ int lbm_set_populations(lbm_grid* g, int l, int which, const double* in) {
   if (!g->bound) return LBM_ESTATE;
   int off, cnt;
   if (pop_range(g, which, &off, &cnt)) return LBM_EINVAL;
+  DeviceScope dev(g->device);
   DevLevel& L = g->dl[l];
   if (L.n == 0) return LBM_OK;
   const long long tot = (long long)L.n * cnt;

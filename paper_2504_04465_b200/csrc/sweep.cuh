@@ -73,6 +73,19 @@ template <typename T, int N> struct alignas(sizeof(T) * N) Vec { T v[N]; };
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// Newton statistics ("mean Newton iterations per update"): two 64-bit counters behind the status word,
+// Newton steps (polish included) and solves; one pair of atomics per warp after a warp-level sum.
+constexpr int NEWTON_COUNTER_OFFSET = 8;      // bytes from the status word
+__device__ __forceinline__ void count_newton(int* status, int it) {
+  const unsigned m = __activemask();
+  const unsigned steps = __reduce_add_sync(m, (unsigned)(it < 0 ? -it - 1 : it));
+  if ((threadIdx.x & 31) == __ffs(m) - 1) {
+    unsigned long long* ctr = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(status) + NEWTON_COUNTER_OFFSET);
+    atomicAdd(ctr, (unsigned long long)steps);
+    atomicAdd(ctr + 1, (unsigned long long)__popc(m));
+  }
+}
+
 // Models whose regular interior is updated through bricks: the polynomial ones (the numerical-equilibrium kernels are
 // fp64-ALU-bound, their list is 9 % of the traffic and their registers are spoken for).
 template <int Q, typename T, int COLL, bool DDF>
@@ -374,6 +387,7 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
     // ---- steps 2-5: moments, equilibrium, sensor, relaxation
     T rho;
     const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f[j], g[j], lam[j], rho, imp);
+    if constexpr (NUMEQ) count_newton(a.status, it);
     if (it < 0) atomicOr(a.status, FLAG_NEWTON);
     if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
 
@@ -465,6 +479,7 @@ __global__ void __launch_bounds__(128) init_kernel(const InitArgs a, const Model
 #pragma unroll
     for (int k = 0; k < NLAMBDA; ++k) { S0[(PL::L0 + k) * a.ps + c] = lam[k]; S1[(PL::L0 + k) * a.ps + c] = lam[k]; }
   }
+  if constexpr (NUMEQ) count_newton(a.status, it);
   if (it < 0) atomicOr(a.status, FLAG_NEWTON);
   T s = T(0);
 #pragma unroll
@@ -529,6 +544,7 @@ __global__ void __launch_bounds__(128) init_coupling_kernel(const CoupleArgs a, 
   }
   T rho;
   const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f, g, lam, rho);
+  if constexpr (NUMEQ) count_newton(a.status, it);
   if (it < 0) atomicOr(a.status, FLAG_NEWTON);
   if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
 #pragma unroll

@@ -14,6 +14,7 @@ LIB_PATH = os.path.join(_HERE, "liblbm_b200.so")
 
 MAX_LEVELS = 24
 BGK, RR, NUMEQ = 0, 1, 2
+ADDR_AUTO, ADDR_LIST, ADDR_BRICKS = 0, 1, 2
 BC_PERIODIC, BC_WALL, BC_MOVING_WALL, BC_INFLOW_VBB, BC_DIRICHLET_EQ, BC_DIRICHLET_EQ_RHO_EXTRAP, BC_NEUMANN = range(7)
 FLUID, FINE_GHOST, COARSE_GHOST, NEUMANN, DIRICHLET = range(5)
 LINK_NONE, LINK_WALL, LINK_VBB0 = -1, -2, -3
@@ -22,9 +23,9 @@ _ERR = {EINVAL: "LBM_EINVAL", ENOMEM: "LBM_ENOMEM", EMESH: "LBM_EMESH", ECUDA: "
         ENEWTON: "LBM_ENEWTON", EUNSUPPORTED: "LBM_EUNSUPPORTED", ESTATE: "LBM_ESTATE"}
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
-SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
+SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_supported_model", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
            "lbm_get_schedule", "lbm_get_sponge", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic", "lbm_get_macroscopic_at",
-           "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_measure_fma_peak"]
+           "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_newton_iterations", "lbm_measure_fma_peak"]
 
 
 class LbmError(RuntimeError):
@@ -43,6 +44,7 @@ class LbmConfig(C.Structure):
         ("bc_rho", C.c_double * 4), ("bc_ux", C.c_double * 4), ("bc_uy", C.c_double * 4), ("bc_T", C.c_double * 4),
         ("sponge_x0", C.c_double), ("sponge_y0", C.c_double), ("sponge_r0", C.c_double), ("sponge_r1", C.c_double),
         ("sponge_sigma_max", C.c_double), ("sponge_rho_inf", C.c_double),
+        ("addressing", C.c_int), ("no_pdl", C.c_int),
     ]
 
 
@@ -72,6 +74,7 @@ def lib():
         L.lbm_destroy.argtypes = [vp]
         L.lbm_destroy.restype = None
         L.lbm_grid_query.argtypes = [vp, C.POINTER(LbmGridInfo)]
+        L.lbm_supported_model.argtypes = [C.c_int, C.POINTER(LbmConfig)]
         L.lbm_get_cells.argtypes = [vp, C.c_int, vp, vp, vp, vp]
         L.lbm_get_nbr.argtypes = [vp, C.c_int, vp]
         L.lbm_get_ghosts.argtypes = [vp, C.c_int, vp, vp, vp]
@@ -93,6 +96,7 @@ def lib():
         L.lbm_last_step_ms.restype = C.c_double
         L.lbm_kernel_name.argtypes = [vp]
         L.lbm_kernel_name.restype = C.c_char_p
+        L.lbm_newton_iterations.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
         L.lbm_measure_fma_peak.argtypes = [C.c_int, C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         _lib = L
     return _lib
@@ -103,6 +107,15 @@ def measure_fma_peak(precision=64, seconds=1.0):
     tf, lm = C.c_double(0.0), C.c_double(0.0)
     _check("lbm_measure_fma_peak", lib().lbm_measure_fma_peak(int(precision), float(seconds), C.byref(tf), C.byref(lm)))
     return tf.value, lm.value
+
+
+def supported_models():
+    """(lattice, precision, collision, ddf, sensor) of every compiled kernel set (lbm_supported_model)."""
+    out, c, i = [], LbmConfig(), 0
+    while lib().lbm_supported_model(i, C.byref(c)) == 0:
+        out.append((c.lattice, c.precision, c.collision, c.ddf, c.sensor))
+        i += 1
+    return out
 
 
 def _ptr(a):
@@ -117,9 +130,10 @@ def _check(where, rc):
 def make_config(lattice=9, precision=64, collision=BGK, ddf=0, sensor=0, trace_eq=0, depth=0, nx_coarse=1, ny_coarse=1,
                 tau0=0.6, T0=0.0, gamma=1.4, sensor_A=1.5, newton_tol=1e-12, newton_max_iter=50,
                 bc=(0, 0, 0, 0), bc_rho=(1, 1, 1, 1), bc_ux=(0, 0, 0, 0), bc_uy=(0, 0, 0, 0), bc_T=(0, 0, 0, 0),
-                sponge=None):
-    """sponge: None or (x0, y0, r0, r1, sigma_max, rho_inf) of Eq. 10-11."""
+                sponge=None, addressing=ADDR_AUTO, no_pdl=0):
+    """sponge: None or (x0, y0, r0, r1, sigma_max, rho_inf) of Eq. 10-11; addressing, no_pdl: device-path options."""
     c = LbmConfig()
+    c.addressing, c.no_pdl = int(addressing), int(no_pdl)
     if sponge is not None:
         (c.sponge_x0, c.sponge_y0, c.sponge_r0, c.sponge_r1, c.sponge_sigma_max, c.sponge_rho_inf) = [float(v) for v in sponge]
     c.lattice, c.precision, c.collision, c.ddf, c.sensor, c.trace_eq = lattice, precision, collision, ddf, sensor, trace_eq
@@ -166,8 +180,9 @@ class Grid:
         self.stream = None
 
     @classmethod
-    def from_case(cls, case, precision=64):
-        kw = case.model_kwargs()
+    def from_case(cls, case, precision=64, **device_options):
+        """device_options: addressing=ADDR_*, no_pdl=0|1 (lbm_config; they never change the result)."""
+        kw = dict(case.model_kwargs(), **device_options)
         if precision == 32:      # Newton tolerance of single-precision runs (P:934: 1e-12 in fp64, 1e-5 in fp32)
             kw["newton_tol"] = max(kw["newton_tol"], 1e-5)
         return cls(make_config(precision=precision, **kw), case.mesh.split, case.mesh.solid)
@@ -267,6 +282,12 @@ class Grid:
 
     def kernel_name(self):
         return lib().lbm_kernel_name(self.h).decode()
+
+    def newton_iterations(self):
+        """(Newton steps, equilibrium solves) counted on the device since bind (lbm_newton_iterations)."""
+        it, ns = C.c_int64(0), C.c_int64(0)
+        _check("lbm_newton_iterations", lib().lbm_newton_iterations(self.h, C.byref(it), C.byref(ns)))
+        return it.value, ns.value
 
     def macroscopic(self, out=None):
         """rho, ux, uy, T of every stored cell; `out` = four caller-owned float64 arrays (e.g. pinned) to fill."""

@@ -25,6 +25,7 @@ BC_PERIODIC, BC_WALL, BC_MOVING_WALL, BC_INFLOW_VBB, BC_DIRICHLET_EQ, BC_DIRICHL
 FLUID, FINE_GHOST, COARSE_GHOST, NEUMANN, DIRICHLET = range(5)
 
 CS2 = {9: 1.0 / 3.0, 13: 0.5, 21: 2.0 / 3.0, 37: 0.697953322019683}   # Table 4 P:815 (used for Mach -> velocity only)
+SOD_T0 = {13: 0.35, 21: 0.9, 37: 1.0}      # inviscid reference temperatures of the numerical equilibria
 
 
 @dataclass
@@ -202,14 +203,18 @@ def cylinder(D=200, depth=5, mach=0.2, re=150.0, seed=1234, collision=RR, lattic
 
 
 # ----------------------------------------------------------------------------- config 4
-def riemann(n=2048, seed=7, lattice=37, periodic=False, sensor=1, tau0=0.5, gamma=1.4, sensor_A=1.5):
+def riemann(n=2048, seed=7, lattice=37, periodic=False, sensor=1, tau0=0.5, gamma=1.4, sensor_A=1.5, collision=BGK, T0=None,
+            mach_max=1.5):
     """Four-quadrant 2-D Riemann problem on a uniform n x n box. Quadrant states are drawn from a seeded
-    generator: rho in [0.5, 8], T/T0 in [0.7, 1.4], |u|/sqrt(gamma T) <= 1.5 (reading S17)."""
+    generator: rho in [0.5, 8], T/T0 in [0.7, 1.4], |u|/sqrt(gamma T) <= mach_max, |u| < 1.9 (reading S17).
+    collision=BGK: the thermal polynomial model of BASELINE configs[3] (T0 = c_s^2); collision=NUMEQ: the numerical
+    equilibrium the paper itself runs on this lattice, reference temperature T0 (default: the inviscid value of
+    P:369)."""
     rng = np.random.RandomState(seed)
-    cs2 = CS2[lattice]
+    Tref = CS2[lattice] if collision != NUMEQ else (SOD_T0[lattice] if T0 is None else T0)
     rho_q = np.exp(rng.uniform(math.log(0.5), math.log(8.0), 4))
-    T_q = cs2 * rng.uniform(0.7, 1.4, 4)
-    ma_q = rng.uniform(0.0, 1.5, 4)
+    T_q = Tref * rng.uniform(0.7, 1.4, 4)
+    ma_q = rng.uniform(0.0, 1.5, 4) * (mach_max / 1.5)
     ang = rng.uniform(0.0, 2 * math.pi, 4)
     sp = np.minimum(ma_q * np.sqrt(gamma * T_q), 1.9)
     ux_q = sp * np.cos(ang); uy_q = sp * np.sin(ang)
@@ -219,15 +224,12 @@ def riemann(n=2048, seed=7, lattice=37, periodic=False, sensor=1, tau0=0.5, gamm
         return rho_q[q], ux_q[q], uy_q[q], T_q[q]
 
     kind = BC_PERIODIC if periodic else BC_NEUMANN
-    return Case("riemann", uniform_mesh(n, n), lattice=lattice, collision=BGK, ddf=1, sensor=sensor, tau0=tau0,
-                gamma=gamma, sensor_A=sensor_A, bc=(kind,) * 4, fields=fields,
+    return Case("riemann", uniform_mesh(n, n), lattice=lattice, collision=collision, ddf=1, sensor=sensor, tau0=tau0,
+                T0=(Tref if collision == NUMEQ else 0.0), gamma=gamma, sensor_A=sensor_A, bc=(kind,) * 4, fields=fields,
                 meta=dict(n=n, rho=rho_q, T=T_q, ux=ux_q, uy=uy_q))
 
 
 # ----------------------------------------------------------------------------- Sod shock tube
-SOD_T0 = {13: 0.35, 21: 0.9, 37: 1.0}      # inviscid reference temperatures
-
-
 def sod(L=8192, lattice=21, mesh="unif", periodic=True, sensor_A=1.5, gamma=1.4, ny=None):
     """Inviscid Sod shock tube (Eq. 12: (p, rho, u) = (10, 8, 0) p0, rho0 left of x = L/2, (1, 1, 0) right) on an
     L x L box (L = finest-equivalent cells per side) with numerical equilibria + g + sensor (A = 1.5), tau = 1/2

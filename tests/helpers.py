@@ -39,10 +39,10 @@ def conserved_sums(g, Q_cx=None, Q_cy=None):
     return np.array([M, PX, PY, E])
 
 
-def gpu_from_case(case, precision=64, init=True):
-    """CUDA-path simulation of the same Case through the C ABI (tests marked gpu)."""
+def gpu_from_case(case, precision=64, init=True, **device_options):
+    """CUDA-path simulation of the same Case through the C ABI (tests marked gpu); device_options: lbm_config.addressing, ..."""
     from paper_2504_04465_b200 import lbm
-    g = lbm.Grid.from_case(case, precision=precision)
+    g = lbm.Grid.from_case(case, precision=precision, **device_options)
     g.bind()
     if init:
         cells = [g.cells(l)[:2] for l in range(g.depth + 1)]

@@ -1,7 +1,7 @@
 """GPU parity of the three addressing modes of the sweep on grids small enough for the oracle
-to follow for many steps: regular bricks forced on small levels (LBM_BRICK_MIN_CELLS=0; by default only levels of
->= 2^18 cells use them, which the full-size tests cover), the default small-level mode (list, one cell per thread),
-and the list-only kernel (LBM_NO_BRICKS=1; fp32: two cells per thread).  The environment is read at bind time."""
+to follow for many steps: regular bricks forced on small levels (lbm_config.addressing = LBM_ADDR_BRICKS; by default
+only levels of >= 2^18 cells use them, which the full-size tests cover), the default small-level mode (list, one cell per
+thread), and the list-only kernel (LBM_ADDR_LIST; fp32: two cells per thread)."""
 import numpy as np
 import pytest
 
@@ -10,7 +10,7 @@ from paper_2504_04465_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-MODES = {"bricks": {"LBM_BRICK_MIN_CELLS": "0"}, "small": {}, "list_only": {"LBM_NO_BRICKS": "1"}}
+MODES = {"bricks": dict(addressing=2), "small": dict(addressing=0), "list_only": dict(addressing=1)}   # LBM_ADDR_*
 TOL = {64: 1e-12, 32: 1e-5}
 
 
@@ -40,17 +40,13 @@ def _cases():
 
 @pytest.mark.parametrize("mode", sorted(MODES))
 @pytest.mark.parametrize("name", sorted(_cases()))
-def test_addressing_modes_match_the_oracle(monkeypatch, name, mode):
+def test_addressing_modes_match_the_oracle(name, mode):
     make, ncoarse = _cases()[name]
     case = make()
-    for k in ("LBM_BRICK_MIN_CELLS", "LBM_NO_BRICKS"):
-        monkeypatch.delenv(k, raising=False)
-    for k, v in MODES[mode].items():
-        monkeypatch.setenv(k, v)
     o = oracle_from_case(case)
     assert o.step(ncoarse) == 0
     for prec in ((64,) if case.ddf else (64, 32)):
-        g = gpu_from_case(case, prec)
+        g = gpu_from_case(case, prec, **MODES[mode])
         if mode == "bricks":
             assert sum(int(g.info.n_bricks[l]) for l in range(g.depth + 1)) > 0
             assert "bricks" in g.kernel_name()
