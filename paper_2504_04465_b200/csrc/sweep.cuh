@@ -76,15 +76,17 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 // Newton statistics ("mean Newton iterations per update"): two 64-bit counters behind the status word,
 // Newton steps (polish included) and solves; one pair of atomics per warp after a warp-level sum.
 constexpr int NEWTON_COUNTER_OFFSET = 8;      // bytes from the status word
-__device__ __forceinline__ void count_newton(int* status, int it) {
+__device__ __forceinline__ void count_newton(int* status, unsigned steps, unsigned solves) {
   const unsigned m = __activemask();
-  const unsigned steps = __reduce_add_sync(m, (unsigned)(it < 0 ? -it - 1 : it));
-  if ((threadIdx.x & 31) == __ffs(m) - 1) {
+  steps = __reduce_add_sync(m, steps);
+  solves = __reduce_add_sync(m, solves);
+  if ((threadIdx.x & 31) == __ffs(m) - 1 && solves != 0u) {
     unsigned long long* ctr = reinterpret_cast<unsigned long long*>(reinterpret_cast<char*>(status) + NEWTON_COUNTER_OFFSET);
     atomicAdd(ctr, (unsigned long long)steps);
-    atomicAdd(ctr + 1, (unsigned long long)__popc(m));
+    atomicAdd(ctr + 1, (unsigned long long)solves);
   }
 }
+__device__ __forceinline__ unsigned newton_steps(int it) { return (unsigned)(it < 0 ? -it - 1 : it); }
 
 // Models whose regular interior is updated through bricks: the polynomial ones (the numerical-equilibrium kernels are
 // fp64-ALU-bound, their list is 9 % of the traffic and their registers are spoken for).
@@ -234,6 +236,7 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
   // (half-way bounce-back), a NONE link the cell's own value (fine ghosts, S6; fixed up below for coarse
   // ghosts), any other link the neighbour's.
   T f[CPT][Q], g[CPT][Q], lam[CPT][NLAMBDA];
+  [[maybe_unused]] unsigned n_steps = 0u, n_solves = 0u;     // Newton statistics, flushed after the stores
 #pragma unroll
   for (int j = 0; j < CPT; ++j) {
     static_for<0, Q>([&](auto ic) {
@@ -387,7 +390,7 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
     // ---- steps 2-5: moments, equilibrium, sensor, relaxation
     T rho;
     const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f[j], g[j], lam[j], rho, imp);
-    if constexpr (NUMEQ) count_newton(a.status, it);
+    if constexpr (NUMEQ) { n_steps += newton_steps(it); n_solves += 1u; }
     if (it < 0) atomicOr(a.status, FLAG_NEWTON);
     if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
 
@@ -438,6 +441,7 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
       for (int j = 0; j < CPT; ++j) o.v[j] = lam[j][k];
       *reinterpret_cast<Vec<T, CPT>*>(Sn + (PL::L0 + k) * ps + c0) = o;
     }
+    count_newton(a.status, n_steps, n_solves);
   }
 }
 
@@ -479,12 +483,12 @@ __global__ void __launch_bounds__(128) init_kernel(const InitArgs a, const Model
 #pragma unroll
     for (int k = 0; k < NLAMBDA; ++k) { S0[(PL::L0 + k) * a.ps + c] = lam[k]; S1[(PL::L0 + k) * a.ps + c] = lam[k]; }
   }
-  if constexpr (NUMEQ) count_newton(a.status, it);
   if (it < 0) atomicOr(a.status, FLAG_NEWTON);
   T s = T(0);
 #pragma unroll
   for (int i = 0; i < Q; ++i) s += f[i];
   if (!(s > T(0)) || !isfinite(s)) atomicOr(a.status, FLAG_UNSTABLE);
+  if constexpr (NUMEQ) count_newton(a.status, newton_steps(it), 1u);
 }
 
 // Coupling of iteration 0 without streaming (listing P:202-208): per coarse ghost, coalesce the unknown
@@ -544,7 +548,6 @@ __global__ void __launch_bounds__(128) init_coupling_kernel(const CoupleArgs a, 
   }
   T rho;
   const int it = collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f, g, lam, rho);
-  if constexpr (NUMEQ) count_newton(a.status, it);
   if (it < 0) atomicOr(a.status, FLAG_NEWTON);
   if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
 #pragma unroll
@@ -571,6 +574,7 @@ __global__ void __launch_bounds__(128) init_coupling_kernel(const CoupleArgs a, 
       for (int k = 0; k < NLAMBDA; ++k) fine[(PL::L0 + k) * a.fps + cj] = lam[k];
     }
   }
+  if constexpr (NUMEQ) count_newton(a.status, newton_steps(it), 1u);
 }
 
 // rho, u, T of every cell of one level from its current populations (Eq. 51)

@@ -216,18 +216,21 @@ def test_unstable_state_is_reported():
 @pytest.mark.parametrize("lattice", [13, 21, 37])
 @pytest.mark.parametrize("mesh", ["unif", "band", "sqr", "hori"])
 def test_sod_numerical_equilibrium_fp64_and_fp32(lattice, mesh):
-    """Numerical equilibria + g + sensor on the paper's four Sod meshes, fp64 (|df| <= 1e-12) and fp32 with the
-    single-precision Newton tolerance of P:934 (|df| <= 1e-5) against the fp64 oracle."""
+    """Numerical equilibria + g + sensor on the paper's four Sod meshes (populations up to 2.8 at rho = 8, Eq. 12): after ONE
+    coarse step north_star's absolute bounds, |df| <= 1e-12 (fp64) and <= 1e-5 (fp32, single-precision Newton tolerance of
+    P:934, against the fp64 oracle); after three coarse steps fp64 still within 1e-12 (measured: <= 3e-14) and fp32 within
+    three times the one-step bound (rounding accumulates step by step; measured: <= 1.4e-5)."""
     case = W.sod(L=64, lattice=lattice, mesh=mesh)
     o = oracle_from_case(case)
-    ncoarse = 3
-    assert o.step(ncoarse) == 0
-    for prec, tol in ((64, 1e-12), (32, 1e-5)):
-        g = gpu_from_case(case, prec)
-        g.step(ncoarse)
-        assert g.sync() == 0
-        d = max_pop_diff(g, o, (0, 1))
-        assert d <= tol * 8.0, (lattice, mesh, prec, d)      # populations scale with rho <= 8 (Eq. 12)
+    gs = {prec: gpu_from_case(case, prec) for prec in (64, 32)}
+    for ncoarse, growth in ((1, 1.0), (2, 3.0)):
+        assert o.step(ncoarse) == 0
+        for prec, g in gs.items():
+            g.step(ncoarse)
+            assert g.sync() == 0
+            d = max_pop_diff(g, o, (0, 1))
+            assert d <= TOL_F[prec] * (growth if prec == 32 else 1.0), (lattice, mesh, prec, ncoarse, d)
+    for g in gs.values():
         g.close()
 
 
