@@ -45,6 +45,7 @@ PAPER_TABLE3 = {(13, "unif"): 1259.1, (13, "hori"): 1088.4, (13, "band"): 1244.8
 REFERENCE_BUDGET_S = 180     # wall-clock cap of the timed region of --impl reference
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
 ADDRESSING = {"auto": 0, "list": 1, "bricks": 2}      # lbm_config.addressing (LBM_ADDR_*)
+PIPELINE = {"auto": 0, "off": 1}                      # lbm_config.pipeline (LBM_PIPE_*): pipelined sweep of the wide models
 # other workloads measured briefly into the default line's `also` (name[@f32|@f64][@list|@bricks])
 DEFAULT_ALSO = "cavity,uniform,cylinder@list,riemann,naca,sod:21:unif@f32"
 KERNEL_SOURCES = ("lattice.cuh", "collide.cuh", "sweep.cuh")
@@ -338,12 +339,16 @@ def newton_block(g, it0, ns0, updates):
 
 def parse_also(entry, precision):
     parts = entry.split("@")
-    opts = dict(precision=precision, addressing="auto")
+    opts = dict(precision=precision, addressing="auto", pipeline="auto", no_prefetch=0)
     for o in parts[1:]:
         if o in ("f32", "f64"):
             opts["precision"] = int(o[1:])
         elif o in ADDRESSING:
             opts["addressing"] = o
+        elif o == "nopipe":
+            opts["pipeline"] = "off"
+        elif o == "noprefetch":
+            opts["no_prefetch"] = 1
         else:
             raise SystemExit("unknown option %r in --also entry %r" % (o, entry))
     return parts[0], opts
@@ -357,7 +362,8 @@ def also_measure(lbm, entry, precision, dev, peak, peak_src):
     case, info = make_case(name, 1.0)
     steps = info.get("also_steps", info["steps"])
     t0 = time.perf_counter()
-    g = lbm.Grid.from_case(case, precision=prec, addressing=ADDRESSING[opts["addressing"]])
+    g = lbm.Grid.from_case(case, precision=prec, addressing=ADDRESSING[opts["addressing"]], pipeline=PIPELINE[opts["pipeline"]],
+                           no_prefetch=opts["no_prefetch"])
     g.bind(dev)
     cells = [g.cells(l)[:2] for l in range(g.depth + 1)]
     rc = g.init_fields(*W.eval_fields(case, cells))
@@ -372,7 +378,7 @@ def also_measure(lbm, entry, precision, dev, peak, peak_src):
     assert status == 0, "device status %d after the timed region of %s" % (status, entry)
     upd = int(g.info.updates_per_coarse_step)
     v = upd * steps / (ms * 1e-3) / 1e6
-    key = "%s_f%d" % (name, prec) + ("" if opts["addressing"] == "auto" else "@" + opts["addressing"])
+    key = "%s_f%d" % (name, prec) + ("" if opts["addressing"] == "auto" else "@" + opts["addressing"]) + ("" if opts["pipeline"] == "auto" else "@nopipe")
     hbm, alu = roofline_blocks(case, prec, g, key, 1.0, v * 1e6, peak, peak_src, fma_peak_of(lbm, prec) if wants_alu(case) else None)
     out = {"workload": info["workload"], "entry": entry, "dtype": "f%d" % prec, "value": v, "unit": "MLUPS", "steps": steps,
            "ms_per_step": ms / steps, "cells": g.ntot, "levels": g.depth + 1, "gpu_launches": int(g.info.launches_per_coarse_step) * steps,
@@ -403,6 +409,9 @@ def main():
     ap.add_argument("--precision", type=int, default=64, choices=[32, 64])
     ap.add_argument("--addressing", default="auto", choices=sorted(ADDRESSING), help="lbm_config.addressing: auto = regular bricks on "
                     "large levels, list = the list-addressed kernel on every level, bricks = bricks on every level")
+    ap.add_argument("--pipeline", default="auto", choices=sorted(PIPELINE), help="lbm_config.pipeline: auto = software-pipelined sweep of "
+                    "the wide models on large levels, off = one cell per thread everywhere")
+    ap.add_argument("--no-prefetch", type=int, default=0, choices=[0, 1], help="lbm_config.no_prefetch (next-wave L2 prefetch of the wide models)")
     ap.add_argument("--scale", type=float, default=1.0, help="linear scale of the workload (1 = BASELINE size)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0, help="0 disables the cpu_baseline leg")
@@ -436,7 +445,8 @@ def main():
         torch.cuda.synchronize()
 
     t_build = time.perf_counter()
-    g = lbm.Grid.from_case(case, precision=args.precision, addressing=ADDRESSING[args.addressing])
+    g = lbm.Grid.from_case(case, precision=args.precision, addressing=ADDRESSING[args.addressing], pipeline=PIPELINE[args.pipeline],
+                           no_prefetch=args.no_prefetch)
     g.bind(dev)
     ntot = g.ntot
     pin = lambda: torch.empty(ntot, dtype=torch.float64).pin_memory().numpy()
@@ -479,7 +489,7 @@ def main():
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e2e_ms = 0.0
     with torch.cuda.stream(g.stream):
-        for it in range(args.e2e_steps + 1):
+        for it in range(args.e2e_steps + 1 if args.e2e_steps > 0 else 0):      # --e2e-steps 0: leg skipped (profiling runs)
             barrier()
             ev0.record(g.stream)
             rc = g.init_fields(*h_in)
@@ -502,7 +512,7 @@ def main():
     mlups = aggregate_mlups(upd, K, world, ms)
     peaks, peak_src = measured_peaks()
     peak = float(peaks.get("hbm_gbs", FALLBACK_HBM_GBS))
-    key = "%s_f%d" % (args.workload, args.precision) + ("" if args.addressing == "auto" else "@" + args.addressing)
+    key = "%s_f%d" % (args.workload, args.precision) + ("" if args.addressing == "auto" else "@" + args.addressing) + ("" if args.pipeline == "auto" else "@nopipe")
     rank_upd_per_s = upd * K / (ms * 1e-3)               # this rank's kernel: every launch of the region is the sweep kernel
     hbm, alu = roofline_blocks(case, args.precision, g, key, args.scale, rank_upd_per_s, peak, peak_src,
                                fma_peak_of(lbm, args.precision) if wants_alu(case) else None)
@@ -520,7 +530,7 @@ def main():
         "metric": "MLUPS (actual cell updates per second)", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K,
         "warmup": args.warmup, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": vs_baseline,
         "dtype": "f%d" % args.precision, "data": "synthetic", "config": config,
-        "kernel": {"name": g.kernel_name(), "addressing": args.addressing, "arena_bytes": int(g.info.arena_bytes),
+        "kernel": {"name": g.kernel_name(), "addressing": args.addressing, "pipeline": args.pipeline, "arena_bytes": int(g.info.arena_bytes),
                    "brick_cell_share": [round(64 * int(g.info.n_bricks[l]) / max(g.n[l], 1), 4) if g.n[l] >= int(g.info.brick_min_level_cells) else 0.0
                                         for l in range(depth + 1)]},
         "mlups": {"actual": mlups, "paper_eq13": n_all * (1 << depth) * K * world / (ms * 1e-3) / 1e6,
@@ -529,9 +539,10 @@ def main():
         "burst": {"steps": kb, "ms_per_step": burst_ms, "value": upd / (burst_ms * 1e-3) / 1e6, "unit": "MLUPS (this rank)",
                   "roofline_frac": upd * hbm["bytes_per_update"] / (burst_ms * 1e-3) / 1e9 / peak,
                   "what": "short region right after warm-up, before the power cap settles"},
-        "e2e": {"value": upd * world / (e2e_ms * 1e-3) / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 4 * 8 * ntot,
-                "d2h_bytes_per_step": 4 * 8 * ntot, "ms_per_step": e2e_ms,
-                "what": "lbm_init_fields (pinned host rho,u,T) + lbm_step(1) + lbm_get_macroscopic (pinned host), every step"},
+        "e2e": None if e2e_ms <= 0 else {
+            "value": upd * world / (e2e_ms * 1e-3) / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": 4 * 8 * ntot,
+            "d2h_bytes_per_step": 4 * 8 * ntot, "ms_per_step": e2e_ms,
+            "what": "lbm_init_fields (pinned host rho,u,T) + lbm_step(1) + lbm_get_macroscopic (pinned host), every step"},
         "gpu_launches": launches * K,
         "clocks": clocks,
         "wall_s_timed_region": wall, "build_s": t_build,

@@ -51,6 +51,8 @@ enum { LBM_FLUID = 0, LBM_FINE_GHOST = 1, LBM_COARSE_GHOST = 2, LBM_NEUMANN = 3,
 enum { LBM_LINK_NONE = -1, LBM_LINK_WALL = -2, LBM_LINK_VBB0 = -3 /* -3-side */ };
 /* device addressing modes (lbm_config.addressing) */
 enum { LBM_ADDR_AUTO = 0, LBM_ADDR_LIST = 1, LBM_ADDR_BRICKS = 2 };
+/* software-pipelined sweep of the wide models (lbm_config.pipeline) */
+enum { LBM_PIPE_AUTO = 0, LBM_PIPE_OFF = 1, LBM_PIPE_ALWAYS = 2 };
 /* error codes */
 enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_EMESH = -3, LBM_ECUDA = -4,
        LBM_EUNSTABLE = -5 /* non-finite or non-positive density */,
@@ -84,9 +86,19 @@ typedef struct {
    * addressing: LBM_ADDR_AUTO = regular 8x8 bricks by tile arithmetic on levels of >= 2^18 stored cells and the neighbour
    * list elsewhere; LBM_ADDR_LIST = the list-addressed kernel of north_star on every level;
    * LBM_ADDR_BRICKS = bricks on every level that has some.  no_pdl = 1: plain stream order between level sweeps instead
-   * of programmatic dependent launch edges. */
+   * of programmatic dependent launch edges.  pipeline: the wide models (second distribution and / or numerical equilibria)
+   * run a software-pipelined persistent sweep (gathers of a thread's next cell in flight as cp.async while it computes the
+   * current one): LBM_PIPE_AUTO = where it was measured faster (D2Q13 fp32 numerical equilibria), on levels
+   * that give every resident thread at least two cells,
+   * LBM_PIPE_OFF = never (one cell per thread everywhere), LBM_PIPE_ALWAYS = on every level.  pipe_max_ctas > 0 caps the
+   * grid of that sweep (default 0: every resident CTA slot of the device), so that threads walk over more cells.
+   * no_prefetch = 1: the one-cell-per-thread sweep of the wide models does not request the next wave's link rows and
+   * population lines into the L2. */
   int addressing;
   int no_pdl;
+  int pipeline;
+  int pipe_max_ctas;
+  int no_prefetch;
 } lbm_config;
 
 typedef struct {

@@ -161,6 +161,85 @@ __device__ __forceinline__ T ipow(T x) {
   else return ipow<N - 1, T>(x) * x;
 }
 
+// Reflection combinations.  Every lattice of Table 4 is symmetric under x -> -x and under y -> -y, and every sum the solver
+// needs is a moment sum_i f_i x^PX y^PY (x^2 + y^2)^PR, which sees only the part of f that is even / odd in x and in y
+// according to the parities of PX and PY.  So the Q values are first combined per reflection orbit -- (a, b), a, b > 0:
+// EE, OE, EO, OO by a two-stage butterfly (8 additions); (a, 0) and (0, b): E, O (2 additions) -- and each moment is then ONE
+// multiply-add per orbit instead of one per direction: D2Q21's 8 residual sums + 16 Jacobian sums take 28 + 41 + 56
+// instructions instead of 113 + 176.  The combination lives in the slot of the orbit member whose signs spell its parities
+// (x < 0: odd in x, y < 0: odd in y).  Only the order of the additions differs from the plain sums.
+// fp64 only: in fp32 the D2Q37 solve sits on its rounding floor (tolerance 1e-5 of P:934 against ~1e-6 rho of summation
+// noise amplified by the Jacobian): re-forming these sums, in this or in any other order, moved the worst cell of the
+// 48^2 parity case from 1.5e-6 to 3.5e-5 of the oracle, so the fp32 kernels keep the plain sums, interleaved with the
+// evaluation of f exactly as before (plain_moment below).
+template <typename T> constexpr bool USE_REFLECT_COMBOS = sizeof(T) == 8;
+
+__host__ __device__ constexpr int dir_index(const LatTab& L, int x, int y) {
+  for (int i = 0; i < L.Q; ++i)
+    if (L.cx[i] == x && L.cy[i] == y) return i;
+  return -1;
+}
+
+template <int Q, typename T>
+__device__ __forceinline__ void reflect_combos(const T (&f)[Q], T (&s)[Q]) {
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I];
+    if constexpr (x == 0 && y == 0) {
+      s[I] = f[I];
+    } else if constexpr ((x > 0 && y == 0) || (x == 0 && y > 0)) {
+      constexpr int J = dir_index(Lat<Q>::t, -x, -y);
+      static_assert(J >= 0, "lattice is not reflection-symmetric");
+      s[I] = f[I] + f[J];
+      s[J] = f[I] - f[J];
+    } else if constexpr (x > 0 && y > 0) {
+      constexpr int Jx = dir_index(Lat<Q>::t, -x, y), Jy = dir_index(Lat<Q>::t, x, -y), Jxy = dir_index(Lat<Q>::t, -x, -y);
+      static_assert(Jx >= 0 && Jy >= 0 && Jxy >= 0, "lattice is not reflection-symmetric");
+      const T p1 = f[I] + f[Jx], m1 = f[I] - f[Jx];      // y = +b row: even / odd in x
+      const T p2 = f[Jy] + f[Jxy], m2 = f[Jy] - f[Jxy];  // y = -b row
+      s[I] = p1 + p2;      // EE
+      s[Jx] = m1 + m2;     // odd in x, even in y
+      s[Jy] = p1 - p2;     // even in x, odd in y
+      s[Jxy] = m1 - m2;    // OO
+    }
+  });
+}
+
+// sum_i f_i x_i^PX y_i^PY (x_i^2 + y_i^2)^PR from the reflection combinations s of f
+template <int Q, typename T, int PX, int PY, int PR>
+__device__ __forceinline__ T sym_moment(const T (&s)[Q]) {
+  T acc = T(0);
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I];
+    constexpr int ax = x < 0 ? -x : x, ay = y < 0 ? -y : y;
+    constexpr bool match = ((PX & 1) == (x < 0 ? 1 : 0)) && ((PY & 1) == (y < 0 ? 1 : 0));
+    constexpr int wgt = ipow_c(ax, PX) * ipow_c(ay, PY) * ipow_c(x * x + y * y, PR);
+    if constexpr (match && wgt != 0) acc += s[I] * T(wgt);
+  });
+  return acc;
+}
+
+// sum_i f_i x_i^PX y_i^PY (x_i^2 + y_i^2)^PR over the directions where the weight is not zero (fp32 kernels)
+template <int Q, typename T, int PX, int PY, int PR>
+__device__ __forceinline__ T plain_moment(const T (&f)[Q]) {
+  T s = T(0);
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I];
+    constexpr int wgt = ipow_c(x, PX) * ipow_c(y, PY) * ipow_c(x * x + y * y, PR);
+    if constexpr (wgt != 0) s += f[I] * T(wgt);
+  });
+  return s;
+}
+
+// the moment from whichever form the precision uses: s = reflection combinations (fp64) or f itself (fp32)
+template <int Q, typename T, int PX, int PY, int PR>
+__device__ __forceinline__ T solver_moment(const T (&s)[Q]) {
+  if constexpr (USE_REFLECT_COMBOS<T>) return sym_moment<Q, T, PX, PY, PR>(s);
+  else return plain_moment<Q, T, PX, PY, PR>(s);
+}
+
 // f_i(lambda) = rho exp[-(1 + sum_a lambda_a M_ia)] (Eq. 39 with a = rho); G_a = sum_i f_i M_ia - m_a.
 // fp32: one expf per direction.  fp64: the lattice velocities are small integers, so the exponential factorises,
 //   f(x,y) = [rho e^{-1-l0}] (e^{-l3})^{x^2} (e^{-l5})^{y^2} (e^{-l4})^{xy} [e^{-l1} (e^{-l6})^{r^2}]^x [e^{-l2} (e^{-l7})^{r^2}]^y,
@@ -169,9 +248,11 @@ __device__ __forceinline__ T ipow(T x) {
 // (profiles/r01_ncu_naca_f64.md).  Each f_i carries a few ulp more rounding error than exp of the summed exponent;
 // the Newton floor stays ~1e-13 rho, below the tolerance of P:934.
 template <int Q, typename T>
-__device__ __forceinline__ void numeq_eval(T rho, const T (&m)[NLAMBDA], const T (&lam)[NLAMBDA], T (&f)[Q], T (&G)[NLAMBDA]) {
+__device__ __forceinline__ void numeq_eval(T rho, const T (&m)[NLAMBDA], const T (&lam)[NLAMBDA], T (&f)[Q], T (&s)[Q], T (&G)[NLAMBDA]) {
+  if constexpr (!USE_REFLECT_COMBOS<T>) {
 #pragma unroll
-  for (int a = 0; a < NLAMBDA; ++a) G[a] = T(0);
+    for (int a = 0; a < NLAMBDA; ++a) G[a] = T(0);
+  }
   [[maybe_unused]] T C, ea, eb, ec, eci, ep, eq, es, et;
   if constexpr (sizeof(T) == 8) {
     C = rho * Num<T>::exp_(-(T(1) + lam[0]));
@@ -209,53 +290,35 @@ __device__ __forceinline__ void numeq_eval(T rho, const T (&m)[NLAMBDA], const T
       fi = rho * Num<T>::exp_(-e);
     }
     f[I] = fi;
-    static_for<0, NLAMBDA>([&](auto ac) {
-      constexpr int A = decltype(ac)::value;
-      constexpr int M = monomial(Lat<Q>::t, I, A);
-      if constexpr (M != 0) G[A] += fi * T(M);
-    });
+    if constexpr (!USE_REFLECT_COMBOS<T>) {
+      static_for<0, NLAMBDA>([&](auto ac) {
+        constexpr int A = decltype(ac)::value;
+        constexpr int M = monomial(Lat<Q>::t, I, A);
+        if constexpr (M != 0) G[A] += fi * T(M);
+      });
+    }
   });
+  if constexpr (!USE_REFLECT_COMBOS<T>) {
 #pragma unroll
-  for (int a = 0; a < NLAMBDA; ++a) G[a] -= m[a];
+    for (int a = 0; a < NLAMBDA; ++a) G[a] -= m[a];
+    return;
+  }
+  // residuals G_a = sum_i f_i M_ia - m_a from the reflection combinations (1, x, y, xx, xy, yy, x r2, y r2)
+  reflect_combos<Q, T>(f, s);
+  G[0] = sym_moment<Q, T, 0, 0, 0>(s) - m[0];
+  G[1] = sym_moment<Q, T, 1, 0, 0>(s) - m[1];
+  G[2] = sym_moment<Q, T, 0, 1, 0>(s) - m[2];
+  G[3] = sym_moment<Q, T, 2, 0, 0>(s) - m[3];
+  G[4] = sym_moment<Q, T, 1, 1, 0>(s) - m[4];
+  G[5] = sym_moment<Q, T, 0, 2, 0>(s) - m[5];
+  G[6] = sym_moment<Q, T, 1, 0, 1>(s) - m[6];
+  G[7] = sym_moment<Q, T, 0, 1, 1>(s) - m[7];
 }
 
-// sum_i f_i x_i^PX y_i^PY (x_i^2 + y_i^2)^PR over the directions where the weight is not zero
-template <int Q, typename T, int PX, int PY, int PR>
-__device__ __forceinline__ T lattice_moment(const T (&f)[Q]) {
-  T s = T(0);
-  static_for<0, Q>([&](auto ic) {
-    constexpr int I = decltype(ic)::value;
-    constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I];
-    constexpr int wgt = ipow_c(x, PX) * ipow_c(y, PY) * ipow_c(x * x + y * y, PR);
-    if constexpr (wgt != 0) s += f[I] * T(wgt);
-  });
-  return s;
-}
-
-// Newton direction: solve (-J) d = G, -J = sum_i f_i M_i M_i^T (symmetric positive definite), by L D L^T.
-// The 36 entries of the lower triangle are 27 distinct lattice moments of f; the eight of the first column are the
-// moment sums the residual already holds (sum_i f_i M_ia = G_a + m_a), three more are sums of two others, so 16 sums
-// over the lattice are formed instead of 36 (the Jacobian was about half of the solve's arithmetic).
-// Returns false if the matrix is not positive definite.
-template <int Q, typename T>
-__device__ __forceinline__ bool newton_direction(const T (&f)[Q], const T (&G)[NLAMBDA], const T (&m)[NLAMBDA], T (&d)[NLAMBDA]) {
-  T A[NLAMBDA][NLAMBDA];   // lower triangle used
-#pragma unroll
-  for (int a = 0; a < NLAMBDA; ++a) A[a][0] = G[a] + m[a];            // 1, x, y, xx, xy, yy, x r2, y r2
-  A[1][1] = A[3][0]; A[2][1] = A[4][0]; A[2][2] = A[5][0];
-  const T xxx = lattice_moment<Q, T, 3, 0, 0>(f), xxy = lattice_moment<Q, T, 2, 1, 0>(f);
-  const T xyy = lattice_moment<Q, T, 1, 2, 0>(f), yyy = lattice_moment<Q, T, 0, 3, 0>(f);
-  const T x4 = lattice_moment<Q, T, 4, 0, 0>(f), x3y = lattice_moment<Q, T, 3, 1, 0>(f), xxyy = lattice_moment<Q, T, 2, 2, 0>(f);
-  const T xy3 = lattice_moment<Q, T, 1, 3, 0>(f), y4 = lattice_moment<Q, T, 0, 4, 0>(f);
-  const T xxr2 = x4 + xxyy, xyr2 = x3y + xy3, yyr2 = xxyy + y4;
-  const T x3r2 = lattice_moment<Q, T, 3, 0, 1>(f), xxyr2 = lattice_moment<Q, T, 2, 1, 1>(f);
-  const T xyyr2 = lattice_moment<Q, T, 1, 2, 1>(f), y3r2 = lattice_moment<Q, T, 0, 3, 1>(f);
-  A[3][1] = xxx; A[4][1] = xxy; A[5][1] = xyy; A[6][1] = xxr2; A[7][1] = xyr2;
-  A[3][2] = xxy; A[4][2] = xyy; A[5][2] = yyy; A[6][2] = xyr2; A[7][2] = yyr2;
-  A[3][3] = x4; A[4][3] = x3y; A[5][3] = xxyy; A[6][3] = x3r2; A[7][3] = xxyr2;
-  A[4][4] = xxyy; A[5][4] = xy3; A[6][4] = xxyr2; A[7][4] = xyyr2;
-  A[5][5] = y4; A[6][5] = xyyr2; A[7][5] = y3r2;
-  A[6][6] = lattice_moment<Q, T, 2, 0, 2>(f); A[7][6] = lattice_moment<Q, T, 1, 1, 2>(f); A[7][7] = lattice_moment<Q, T, 0, 2, 2>(f);
+// Solves A d = G for a symmetric positive definite 8x8 A given by its lower triangle, by L D L^T in place; false if a
+// pivot is not positive.
+template <typename T>
+__device__ __forceinline__ bool ldlt_solve(T (&A)[NLAMBDA][NLAMBDA], const T (&G)[NLAMBDA], T (&d)[NLAMBDA]) {
   // A = L D L^T in place (unit lower L below the diagonal, D on it): the square-root-free form of the Cholesky
   // factorisation -- the same direction up to rounding, but each column waits for one refined reciprocal (5 dependent
   // instructions) instead of a square root and a division (~40), which matters with two warps per scheduler.
@@ -296,6 +359,33 @@ __device__ __forceinline__ bool newton_direction(const T (&f)[Q], const T (&G)[N
   return ok;
 }
 
+// Newton direction: solve (-J) d = G, -J = sum_i f_i M_i M_i^T (symmetric positive definite), by L D L^T.
+// The 36 entries of the lower triangle are 27 distinct lattice moments of f; the eight of the first column are the
+// moment sums the residual already holds (sum_i f_i M_ia = G_a + m_a), three more are sums of two others, so 16 sums
+// over the lattice are formed instead of 36 (the Jacobian was about half of the solve's arithmetic).
+// Returns false if the matrix is not positive definite.
+template <int Q, typename T>
+__device__ __forceinline__ bool newton_direction(const T (&f)[Q], const T (&G)[NLAMBDA], const T (&m)[NLAMBDA], T (&d)[NLAMBDA]) {   // f: reflection combinations (fp64) or f itself (fp32)
+  T A[NLAMBDA][NLAMBDA];   // lower triangle used
+#pragma unroll
+  for (int a = 0; a < NLAMBDA; ++a) A[a][0] = G[a] + m[a];            // 1, x, y, xx, xy, yy, x r2, y r2
+  A[1][1] = A[3][0]; A[2][1] = A[4][0]; A[2][2] = A[5][0];
+  const T xxx = solver_moment<Q, T, 3, 0, 0>(f), xxy = solver_moment<Q, T, 2, 1, 0>(f);
+  const T xyy = solver_moment<Q, T, 1, 2, 0>(f), yyy = solver_moment<Q, T, 0, 3, 0>(f);
+  const T x4 = solver_moment<Q, T, 4, 0, 0>(f), x3y = solver_moment<Q, T, 3, 1, 0>(f), xxyy = solver_moment<Q, T, 2, 2, 0>(f);
+  const T xy3 = solver_moment<Q, T, 1, 3, 0>(f), y4 = solver_moment<Q, T, 0, 4, 0>(f);
+  const T xxr2 = x4 + xxyy, xyr2 = x3y + xy3, yyr2 = xxyy + y4;
+  const T x3r2 = solver_moment<Q, T, 3, 0, 1>(f), xxyr2 = solver_moment<Q, T, 2, 1, 1>(f);
+  const T xyyr2 = solver_moment<Q, T, 1, 2, 1>(f), y3r2 = solver_moment<Q, T, 0, 3, 1>(f);
+  A[3][1] = xxx; A[4][1] = xxy; A[5][1] = xyy; A[6][1] = xxr2; A[7][1] = xyr2;
+  A[3][2] = xxy; A[4][2] = xyy; A[5][2] = yyy; A[6][2] = xyr2; A[7][2] = yyr2;
+  A[3][3] = x4; A[4][3] = x3y; A[5][3] = xxyy; A[6][3] = x3r2; A[7][3] = xxyr2;
+  A[4][4] = xxyy; A[5][4] = xy3; A[6][4] = xxyr2; A[7][4] = xyyr2;
+  A[5][5] = y4; A[6][5] = xyyr2; A[7][5] = y3r2;
+  A[6][6] = solver_moment<Q, T, 2, 0, 2>(f); A[7][6] = solver_moment<Q, T, 1, 1, 2>(f); A[7][7] = solver_moment<Q, T, 0, 2, 2>(f);
+  return ldlt_solve<T>(A, G, d);
+}
+
 template <typename T>
 __device__ __forceinline__ T norm2sq(const T (&G)[NLAMBDA]) {
   T s = T(0);
@@ -304,11 +394,162 @@ __device__ __forceinline__ T norm2sq(const T (&G)[NLAMBDA]) {
   return s;
 }
 
+// ---- fp64: the solve in one pass per trial point.  The 8 residual sums and the 16 further lattice moments of the
+// Jacobian are accumulated orbit by orbit while the f_i of the trial point are formed (rest; (+-a, 0); (0, +-a);
+// (+-a, +-b) through the reflection combinations above), so that no array of Q equilibrium values (nor of their
+// combinations) is live across the factorisation: the kernels sat at 254-255 registers with spills, the f_i of the
+// final point are evaluated once more after the loop instead (products of the 8 exponentials only, no sums), which also
+// replaces the polish phase's full evaluation.  Same rule (S14), same phases, same tests as the loop below.
+constexpr int NSUM = 24;
+//                                 G: 1  x  y  xx xy yy xr2 yr2 | xxx xxy xyy yyy x4 x3y xxyy xy3 y4 x3r2 xxyr2 xyyr2 y3r2 xxr4 xyr4 yyr4
+__device__ constexpr int SUM_PX[NSUM] = {0, 1, 0, 2, 1, 0, 1, 0, 3, 2, 1, 0, 4, 3, 2, 1, 0, 3, 2, 1, 0, 2, 1, 0};
+__device__ constexpr int SUM_PY[NSUM] = {0, 0, 1, 0, 1, 2, 0, 1, 0, 1, 2, 3, 0, 1, 2, 3, 4, 0, 1, 2, 3, 0, 1, 2};
+__device__ constexpr int SUM_PR[NSUM] = {0, 0, 0, 0, 0, 0, 1, 1, 0, 0, 0, 0, 0, 0, 0, 0, 0, 1, 1, 1, 1, 2, 2, 2};
+
+struct NumeqExps { double C, ea, eb, ec, eci, ep, eq, es, et; };
+
+__device__ __forceinline__ void numeq_exps(double rho, const double (&lam)[NLAMBDA], NumeqExps& E) {
+  E.C = rho * exp(-(1.0 + lam[0]));
+  E.ep = exp(-lam[1]); E.eq = exp(-lam[2]);
+  E.ea = exp(-lam[3]); E.ec = exp(-lam[4]); E.eb = exp(-lam[5]);
+  E.es = exp(-lam[6]); E.et = exp(-lam[7]);
+  E.eci = fast_rcp(E.ec);
+}
+
+// f_I from the factorised exponentials (see numeq_eval)
+template <int Q, int I>
+__device__ __forceinline__ double numeq_f(const NumeqExps& E) {
+  constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I], r2 = x * x + y * y;
+  constexpr int ax = x < 0 ? -x : x, ay = y < 0 ? -y : y, axy = x * y < 0 ? -x * y : x * y;
+  double fi = E.C;
+  if constexpr (x != 0) fi *= ipow<x * x, double>(E.ea);
+  if constexpr (y != 0) fi *= ipow<y * y, double>(E.eb);
+  if constexpr (x * y > 0) fi *= ipow<axy, double>(E.ec);
+  if constexpr (x * y < 0) fi *= ipow<axy, double>(E.eci);
+  if constexpr (x != 0) {
+    const double X = ipow<ax, double>(E.ep * ipow<r2, double>(E.es));
+    fi *= x > 0 ? X : fast_rcp(X);
+  }
+  if constexpr (y != 0) {
+    const double Y = ipow<ay, double>(E.eq * ipow<r2, double>(E.et));
+    fi *= y > 0 ? Y : fast_rcp(Y);
+  }
+  return fi;
+}
+
+// adds the reflection combination v that lives in slot I (parities spelled by the signs of xi_I) to every sum it enters
+template <int Q, int I>
+__device__ __forceinline__ void numeq_accumulate(double v, double (&S)[NSUM]) {
+  constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I];
+  constexpr int ax = x < 0 ? -x : x, ay = y < 0 ? -y : y;
+  static_for<0, NSUM>([&](auto kc) {
+    constexpr int K = decltype(kc)::value;
+    constexpr bool match = ((SUM_PX[K] & 1) == (x < 0 ? 1 : 0)) && ((SUM_PY[K] & 1) == (y < 0 ? 1 : 0));
+    constexpr int wgt = ipow_c(ax, SUM_PX[K]) * ipow_c(ay, SUM_PY[K]) * ipow_c(x * x + y * y, SUM_PR[K]);
+    if constexpr (match && wgt != 0) S[K] += v * double(wgt);
+  });
+}
+
+template <int Q>
+__device__ __forceinline__ void numeq_pass(double rho, const double (&lam)[NLAMBDA], double (&S)[NSUM]) {
+  NumeqExps E;
+  numeq_exps(rho, lam, E);
+#pragma unroll
+  for (int k = 0; k < NSUM; ++k) S[k] = 0.0;
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int x = Lat<Q>::t.cx[I], y = Lat<Q>::t.cy[I];
+    if constexpr (x == 0 && y == 0) {
+      numeq_accumulate<Q, I>(numeq_f<Q, I>(E), S);
+    } else if constexpr ((x > 0 && y == 0) || (x == 0 && y > 0)) {
+      constexpr int J = dir_index(Lat<Q>::t, -x, -y);
+      const double fp = numeq_f<Q, I>(E), fm = numeq_f<Q, J>(E);
+      numeq_accumulate<Q, I>(fp + fm, S);
+      numeq_accumulate<Q, J>(fp - fm, S);
+    } else if constexpr (x > 0 && y > 0) {
+      constexpr int Jx = dir_index(Lat<Q>::t, -x, y), Jy = dir_index(Lat<Q>::t, x, -y), Jxy = dir_index(Lat<Q>::t, -x, -y);
+      const double f1 = numeq_f<Q, I>(E), f2 = numeq_f<Q, Jx>(E), f3 = numeq_f<Q, Jy>(E), f4 = numeq_f<Q, Jxy>(E);
+      const double p1 = f1 + f2, m1 = f1 - f2, p2 = f3 + f4, m2 = f3 - f4;
+      numeq_accumulate<Q, I>(p1 + p2, S);
+      numeq_accumulate<Q, Jx>(m1 + m2, S);
+      numeq_accumulate<Q, Jy>(p1 - p2, S);
+      numeq_accumulate<Q, Jxy>(m1 - m2, S);
+    }
+  });
+}
+
+__device__ __forceinline__ bool newton_direction_from_sums(const double (&S)[NSUM], const double (&G)[NLAMBDA], double (&d)[NLAMBDA]) {
+  double A[NLAMBDA][NLAMBDA];   // lower triangle of -J = sum_i f_i M_i M_i^T
+#pragma unroll
+  for (int a = 0; a < NLAMBDA; ++a) A[a][0] = S[a];
+  A[1][1] = S[3]; A[2][1] = S[4]; A[2][2] = S[5];
+  const double xxx = S[8], xxy = S[9], xyy = S[10], yyy = S[11], x4 = S[12], x3y = S[13], xxyy = S[14], xy3 = S[15], y4 = S[16];
+  const double xxr2 = x4 + xxyy, xyr2 = x3y + xy3, yyr2 = xxyy + y4;
+  const double x3r2 = S[17], xxyr2 = S[18], xyyr2 = S[19], y3r2 = S[20];
+  A[3][1] = xxx; A[4][1] = xxy; A[5][1] = xyy; A[6][1] = xxr2; A[7][1] = xyr2;
+  A[3][2] = xxy; A[4][2] = xyy; A[5][2] = yyy; A[6][2] = xyr2; A[7][2] = yyr2;
+  A[3][3] = x4; A[4][3] = x3y; A[5][3] = xxyy; A[6][3] = x3r2; A[7][3] = xxyr2;
+  A[4][4] = xxyy; A[5][4] = xy3; A[6][4] = xxyr2; A[7][4] = xyyr2;
+  A[5][5] = y4; A[6][5] = xyyr2; A[7][5] = y3r2;
+  A[6][6] = S[21]; A[7][6] = S[22]; A[7][7] = S[23];
+  return ldlt_solve<double>(A, G, d);
+}
+
+template <int Q>
+__device__ __forceinline__ int feq_numerical_onepass(const ModelParams& p, double rho, double ux, double uy, double Tm,
+                                                     double (&lam)[NLAMBDA], double (&f)[Q]) {
+  const double u2 = ux * ux + uy * uy;
+  const double m[NLAMBDA] = {rho, rho * ux, rho * uy, rho * (ux * ux + Tm), rho * ux * uy, rho * (uy * uy + Tm),
+                             rho * ux * (u2 + 4.0 * Tm), rho * uy * (u2 + 4.0 * Tm)};
+  double S[NSUM], G[NLAMBDA], d[NLAMBDA], lt[NLAMBDA];
+  const double tol = p.newton_tol * rho;
+  enum { INIT, SEARCH, POLISH };
+  int it = 0, phase = INIT;
+  bool converged = false, bad = false;
+  double t = 0.0, n0 = 0.0;
+#pragma unroll
+  for (int a = 0; a < NLAMBDA; ++a) d[a] = 0.0;
+#pragma unroll 1
+  for (;;) {
+#pragma unroll
+    for (int a = 0; a < NLAMBDA; ++a) lt[a] = lam[a] + t * d[a];
+    if (phase == POLISH) {        // the unconditional full step; its equilibrium is evaluated below
+#pragma unroll
+      for (int a = 0; a < NLAMBDA; ++a) lam[a] = lt[a];
+      ++it;
+      break;
+    }
+    numeq_pass<Q>(rho, lt, S);
+#pragma unroll
+    for (int a = 0; a < NLAMBDA; ++a) G[a] = S[a] - m[a];
+    if (phase == SEARCH) {
+      const double n1 = norm2sq(G);
+      if (!(n1 < n0) && t > 1.0 / 1024.0) { t *= 0.5; continue; }   // a NaN norm keeps halving
+    }
+#pragma unroll
+    for (int a = 0; a < NLAMBDA; ++a) lam[a] = lt[a];
+    if (phase != INIT) ++it;
+    double r1 = 0.0;
+#pragma unroll
+    for (int a = 0; a < NLAMBDA; ++a) r1 += fabs(G[a]);
+    converged = r1 <= tol;
+    phase = (converged || it >= p.newton_max_iter) ? POLISH : SEARCH;
+    if (!newton_direction_from_sums(S, G, d)) { bad = true; break; }
+    n0 = norm2sq(G);
+    t = 1.0;
+  }
+  NumeqExps E;
+  numeq_exps(rho, lam, E);
+  static_for<0, Q>([&](auto ic) { f[decltype(ic)::value] = numeq_f<Q, decltype(ic)::value>(E); });
+  return (converged && !bad) ? it : -it - 1;
+}
+
 // Newton-Raphson with a halving line search; deterministic rule of DESIGN.md Sec. 4 (S14):
 // iterate until sum|G_a| <= tol*rho or max_iter, then one unconditional full Newton step.
 // lam in/out; feq out.  Returns the number of Newton steps (polish included), negative on failure.
 template <int Q, typename T>
 __device__ __forceinline__ int feq_numerical(const ModelParams& p, T rho, T ux, T uy, T Tm, T (&lam)[NLAMBDA], T (&f)[Q]) {
+  if constexpr (sizeof(T) == 8) return feq_numerical_onepass<Q>(p, rho, ux, uy, Tm, lam, f);
   const T u2 = ux * ux + uy * uy;
   // right-hand sides of Eq. 42-49 with 2E = u^2 + 2T
   const T m[NLAMBDA] = {rho, rho * ux, rho * uy, rho * (ux * ux + Tm), rho * ux * uy, rho * (uy * uy + Tm),
@@ -317,6 +558,7 @@ __device__ __forceinline__ int feq_numerical(const ModelParams& p, T rho, T ux, 
   // initial residual, line-search trial, polish -- are phases of it): fully inlined, each site is ~1-2 k instructions,
   // and three copies of them overflowed the instruction cache (profiles/r01_ncu_naca_f64.md: stall_no_instruction).
   T G[NLAMBDA], d[NLAMBDA], lt[NLAMBDA];
+  [[maybe_unused]] T sc[Q];        // reflection combinations of the trial equilibrium (fp64)
   const T tol = T(p.newton_tol) * rho;
   enum { INIT, SEARCH, POLISH };
   int it = 0, phase = INIT;
@@ -328,7 +570,7 @@ __device__ __forceinline__ int feq_numerical(const ModelParams& p, T rho, T ux, 
   for (;;) {
 #pragma unroll
     for (int a = 0; a < NLAMBDA; ++a) lt[a] = lam[a] + t * d[a];
-    numeq_eval<Q, T>(rho, m, lt, f, G);
+    numeq_eval<Q, T>(rho, m, lt, f, sc, G);
     if (phase == SEARCH) {
       const T n1 = norm2sq(G);
       if (!(n1 < n0) && t > T(1.0 / 1024.0)) { t *= T(0.5); continue; }   // a NaN norm keeps halving
@@ -342,7 +584,7 @@ __device__ __forceinline__ int feq_numerical(const ModelParams& p, T rho, T ux, 
     for (int a = 0; a < NLAMBDA; ++a) r1 += Num<T>::abs_(G[a]);
     converged = r1 <= tol;
     phase = (converged || it >= p.newton_max_iter) ? POLISH : SEARCH;    // then one unconditional full Newton step
-    if (!newton_direction<Q, T>(f, G, m, d)) { bad = true; break; }
+    if (!newton_direction<Q, T>(USE_REFLECT_COMBOS<T> ? sc : f, G, m, d)) { bad = true; break; }
     n0 = norm2sq(G);
     t = T(1);
   }

@@ -74,6 +74,10 @@ struct lbm_grid {
   size_t off_tab = 0;
   unsigned short* d_tab = nullptr;
   bool pdl = true;                                // programmatic dependent launch between level sweeps (lbm_config.no_pdl)
+  int pf_dist = 0;                                // next-wave L2 prefetch distance of the one-cell-per-thread sweep of the wide models (cells)
+  bool pipe = false;                              // software-pipelined persistent sweep on large levels (sweep_pipe.cuh)
+  int pipe_grid = 0;                              // resident CTAs of the pipelined sweep on this device (occupancy x SMs)
+  int64_t pipe_min_cells = 0;                     // levels below this keep one cell per thread
   char* arena = nullptr;
   cudaStream_t stream = nullptr;
   int* d_status = nullptr;
@@ -126,7 +130,7 @@ const KernelSet* find_kernel_set(const lbm_config& c) {
 
 // n work items, `per_thread` of them per thread.  pdl: chain to the previous kernel of the stream with a programmatic
 // dependent-launch edge (only for kernels that call griddepcontrol.wait before touching mutable data: the sweep).
-int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem = 0);
+int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem = 0, int block = BLOCK);
 
 int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s, int per_thread = 1, bool pdl = false, int smem = 0) {
   if (n <= 0) return LBM_OK;
@@ -134,15 +138,15 @@ int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s, int pe
   return launch_grid(fn, (unsigned)((threads + BLOCK - 1) / BLOCK), a0, a1, s, pdl, smem);
 }
 
-int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem) {
+int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem, int block) {
   if (grid == 0) return LBM_OK;
   void* args[2] = {a0, a1};
   if (!pdl) {
-    CK(cudaLaunchKernel(fn, dim3(grid), dim3(BLOCK), args, (size_t)smem, s));
+    CK(cudaLaunchKernel(fn, dim3(grid), dim3((unsigned)block), args, (size_t)smem, s));
     return LBM_OK;
   }
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(grid); cfg.blockDim = dim3(BLOCK); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = s;
+  cfg.gridDim = dim3(grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = s;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -165,6 +169,7 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   a.sigma = L.sigma;
   a.brick_nb = L.brick_nb; a.brick_tab = g->d_tab; a.irr = L.irr;
   a.nbrick = (int)L.nbrick; a.n_irr = (int)L.n_irr;
+  a.n_inbox = (int)g->hg.lv[l].n_inbox; a.pf_dist = 0;
   const int64_t cells_per_cta = g->ks->brick_cells_per_cta;
   a.brick_ctas = (int)((L.nbrick * 64 + cells_per_cta - 1) / cells_per_cta);
   a.list_ctas = (int)((L.n_irr + BLOCK - 1) / BLOCK);
@@ -172,13 +177,20 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   // of the brick kernel with no bricks and no indirection), which gives them the most threads; measured on the 39 k-cell
   // cavity: fp64 7.4 against 6.6 GLUPS with bricks (two cells per thread).
   int rc;
-  if (g->bricks && L.n < g->brick_min_cells) {
+  if (g->pipe && L.n >= g->pipe_min_cells) {
+    // wide models, large level: persistent grid (every resident CTA slot of the device once), each thread walks over
+    // n / (grid * block) cells with the next cell's gathers in flight
+    const int tpb = g->ks->pipe_tpb;
+    const int64_t ctas = std::min<int64_t>(g->pipe_grid, (L.n + tpb - 1) / tpb);
+    rc = launch_grid(g->ks->sweep_pipe, (unsigned)ctas, &a, &g->mp, g->stream, g->pdl, g->ks->pipe_smem, tpb);
+  } else if (g->bricks && L.n < g->brick_min_cells) {
     a.nbrick = 0; a.brick_ctas = 0; a.irr = nullptr; a.n_irr = (int)L.n;
     a.list_ctas = (int)((L.n + BLOCK - 1) / BLOCK);
     rc = launch_grid(g->ks->sweep_bricks, (unsigned)a.list_ctas, &a, &g->mp, g->stream, g->pdl);
   } else if (g->bricks && L.nbrick > 0) {
     rc = launch_grid(g->ks->sweep_bricks, (unsigned)(a.list_ctas + a.brick_ctas), &a, &g->mp, g->stream, g->pdl);
   } else {
+    if (L.n >= 4ll * g->pf_dist) a.pf_dist = g->pf_dist;      // smaller levels live in the L2 anyway
     rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream, g->ks->cells_per_thread, g->pdl);
   }
   if (rc == LBM_OK) cur[l] ^= 1;
@@ -245,6 +257,7 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
   if (cfg->collision == LBM_RR && cfg->ddf) return LBM_EINVAL;     // RR is defined for the athermal models only
   if (!(cfg->tau0 >= 0.5)) return LBM_EINVAL;
   if (cfg->addressing < LBM_ADDR_AUTO || cfg->addressing > LBM_ADDR_BRICKS) return LBM_EINVAL;
+  if (cfg->pipeline < LBM_PIPE_AUTO || cfg->pipeline > LBM_PIPE_ALWAYS || cfg->pipe_max_ctas < 0) return LBM_EINVAL;
   // the sponge relaxes rho = p / T0: weakly compressible models only
   if (cfg->sponge_sigma_max != 0.0 && (cfg->ddf || cfg->collision == LBM_NUMEQ || !(cfg->sponge_sigma_max > 0.0) ||
                                        !(cfg->sponge_sigma_max <= 1.0) || !(cfg->sponge_r1 > cfg->sponge_r0) || !(cfg->sponge_r0 >= 0.0)))
@@ -270,6 +283,7 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
     g->bricks = ks->sweep_bricks != nullptr && cfg->addressing != LBM_ADDR_LIST;
     g->brick_min_cells = !g->bricks ? INT64_MAX : cfg->addressing == LBM_ADDR_BRICKS ? 0 : BRICK_MIN_LEVEL_CELLS;
     g->pdl = cfg->no_pdl == 0;
+    g->pipe = ks->sweep_pipe != nullptr && (cfg->pipeline == LBM_PIPE_ALWAYS || (cfg->pipeline == LBM_PIPE_AUTO && ks->pipe_auto));
     ModelParams& mp = g->mp;
     mp.gamma = cfg->gamma; mp.sensor_A = cfg->sensor_A; mp.T0 = cfg->T0; mp.newton_tol = cfg->newton_tol;
     mp.newton_max_iter = cfg->newton_max_iter; mp.trace_eq = cfg->trace_eq;
@@ -467,6 +481,26 @@ int bind_impl(lbm_grid* g, void* dev_arena, void* cuda_stream) {
   CK(cudaStreamSynchronize(g->stream));
   CK(cudaEventCreate(&g->ev0));
   CK(cudaEventCreate(&g->ev1));
+  if ((g->hg.cfg.ddf || g->hg.cfg.collision == LBM_NUMEQ) && g->hg.cfg.no_prefetch == 0) {
+    // wide models: distance of the next-wave L2 prefetch = the cells one wave of resident CTAs covers
+    int per_sm = 0, sms = 0;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, g->ks->sweep, BLOCK, 0));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device));
+    g->pf_dist = per_sm * sms * BLOCK * g->ks->cells_per_thread;
+  }
+  if (g->pipe) {
+    // the pipelined sweep stages two cells per thread in shared memory (opt-in above 48 KB) and is launched as ONE wave:
+    // grid = resident CTAs per SM (registers and shared memory decide) x SMs of this device
+    int per_sm = 0, sms = 0;
+    CK(cudaFuncSetAttribute(g->ks->sweep_pipe, cudaFuncAttributeMaxDynamicSharedMemorySize, g->ks->pipe_smem));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, g->ks->sweep_pipe, g->ks->pipe_tpb, (size_t)g->ks->pipe_smem));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device));
+    if (per_sm < 1 || sms < 1) return LBM_ECUDA;
+    g->pipe_grid = per_sm * sms;
+    if (g->hg.cfg.pipe_max_ctas > 0) g->pipe_grid = std::min(g->pipe_grid, g->hg.cfg.pipe_max_ctas);
+    // a level must give every thread at least two cells for the prefetch to overlap anything
+    g->pipe_min_cells = g->hg.cfg.pipeline == LBM_PIPE_ALWAYS ? 0 : 2ll * g->pipe_grid * g->ks->pipe_tpb;
+  }
   // graphs (one coarse step from either parity of the coarsest level; K steps for launch-bound grids) are captured on
   // first use by lbm_step and dropped when a parameter baked into their kernel arguments changes
   g->K = 0;
@@ -680,7 +714,7 @@ int lbm_newton_iterations(lbm_grid* g, int64_t* iterations, int64_t* solves) {
 
 const char* lbm_kernel_name(const lbm_grid* g) {
   if (!g) return "";
-  return g->bricks ? g->ks->bricks_name : g->ks->name;
+  return (g->pipe && g->hg.lv[0].n >= g->pipe_min_cells) ? g->ks->pipe_name : g->bricks ? g->ks->bricks_name : g->ks->name;
 }
 
 int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double* T) {

@@ -46,6 +46,8 @@ struct LevelArgs {
   const unsigned short* brick_tab;   // [(Q-1)][64] (k << 6) | Z-position of the pull source
   const int* irr;
   int nbrick, n_irr, brick_ctas, list_ctas;
+  int n_inbox;              // cells [n_inbox, n) are the boundary cells (Neumann / Dirichlet), the only ones that read aux early
+  int pf_dist;              // L2 prefetch distance in cells (one wave of resident CTAs ahead), 0 = off
 };
 
 template <int Q, bool DDF, int COLL>
@@ -72,6 +74,7 @@ template <typename T, int N> struct alignas(sizeof(T) * N) Vec { T v[N]; };
 // ghost rows) before waiting for this sweep's memory to be visible.
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // Newton statistics ("mean Newton iterations per update"): two 64-bit counters behind the status word,
 // Newton steps (polish included) and solves; one pair of atomics per warp after a warp-level sum.
@@ -210,23 +213,25 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
   // handled as a link-less fine ghost (it moves padding to padding).
   int type[CPT], side[CPT], self[CPT], nb[CPT][Q];
   {
+    // every index load is issued before any is used: the type byte, the links and (boundary cells only, known from the
+    // storage order) the source cell arrive together, one DRAM round trip in front of the gathers instead of two
     const Vec<unsigned char, CPT> tv = *reinterpret_cast<const Vec<unsigned char, CPT>*>(a.type + c0);
-#pragma unroll
-    for (int j = 0; j < CPT; ++j) {
-      const bool valid = c0 + j < a.n;
-      type[j] = valid ? (tv.v[j] & TYPE_MASK) : LBM_FINE_GHOST;
-      side[j] = tv.v[j] >> TYPE_SIDE_SHIFT;
-    }
     static_for<1, Q>([&](auto ic) {
       constexpr int I = decltype(ic)::value;
       const Vec<int, CPT> nv = *reinterpret_cast<const Vec<int, CPT>*>(a.nbr + (long long)(I - 1) * ps + c0);
 #pragma unroll
       for (int j = 0; j < CPT; ++j) nb[j][I] = (c0 + j < a.n) ? nv.v[j] : LBM_LINK_NONE;
     });
+    int src_cell[CPT];
+#pragma unroll
+    for (int j = 0; j < CPT; ++j) src_cell[j] = (c0 + j >= a.n_inbox && c0 + j < a.n) ? a.aux[c0 + j] : c0 + j;
 #pragma unroll
     for (int j = 0; j < CPT; ++j) {
+      const bool valid = c0 + j < a.n;
+      type[j] = valid ? (tv.v[j] & TYPE_MASK) : LBM_FINE_GHOST;
+      side[j] = tv.v[j] >> TYPE_SIDE_SHIFT;
       // a NEUMANN cell replicates the complete update of its source cell (reading S13)
-      self[j] = (type[j] == LBM_NEUMANN) ? a.aux[c0 + j] : c0 + j;
+      self[j] = (type[j] == LBM_NEUMANN) ? src_cell[j] : c0 + j;
       nb[j][0] = self[j];
     }
   }
@@ -248,6 +253,22 @@ __global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep
       f[j][I] = So[comp * ps + src];
       if constexpr (DDF) g[j][I] = So[(PL::G0 + comp) * ps + src];
     });
+  }
+
+  // ---- next wave into L2.  A wide model keeps 8-12 warps per SM, too few to hide the two dependent DRAM round trips
+  // (links, then gathers) in front of its arithmetic (profiles/r02_ncu_naca_f64.md: stall_long_scoreboard 2.5 per issue,
+  // 44 % of the samples).  The CTAs that follow this one on its SM slot work pf_dist cells further along the Z-curve:
+  // their link rows, and the population lines at their own indices (which hold most of their neighbours: the gathers of 128
+  // consecutive Morton cells fall into the same few lines per plane), are requested now, so that their round trips end
+  // in the L2.  Every line is still fetched from DRAM once; a prefetch that misses its target is only wasted.
+  if (a.pf_dist > 0) {
+    const long long cp = (long long)c0 + a.pf_dist;
+    if (cp < a.n) {
+      prefetch_l2(a.type + cp);
+      static_for<1, Q>([&](auto ic) { prefetch_l2(a.nbr + (long long)(decltype(ic)::value - 1) * ps + cp); });
+#pragma unroll
+      for (int q = 0; q < PL::NPOP; ++q) prefetch_l2(So + q * ps + cp);
+    }
   }
 
 #pragma unroll
@@ -618,6 +639,11 @@ struct KernelSet {
   const void* init;
   const void* couple;
   const void* macro;
+  // software-pipelined persistent sweep of the wide models (sweep_pipe.cuh), or null
+  const void* sweep_pipe;
+  const char* pipe_name;
+  int pipe_tpb, pipe_smem;
+  int pipe_auto;            // 1: LBM_PIPE_AUTO selects it on large levels (measured faster than one cell per thread)
 };
 
 template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
@@ -634,6 +660,7 @@ KernelSet make_kernel_set(const char* name, const char* bricks_name) {
   k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;
   k.couple = (const void*)&init_coupling_kernel<Q, T, COLL, DDF, SENSOR>;
   k.macro = (const void*)&macroscopic_kernel<Q, T, COLL, DDF>;
+  k.sweep_pipe = nullptr; k.pipe_name = ""; k.pipe_tpb = 0; k.pipe_smem = 0; k.pipe_auto = 0;
   return k;
 }
 

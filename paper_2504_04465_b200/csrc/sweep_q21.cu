@@ -1,6 +1,6 @@
 // sweep_q21.cu -- D2Q21 instantiations of the level-sweep kernels (sweep.cuh); one translation unit per
 // lattice so that the instantiations compile in parallel.
-#include "sweep.cuh"
+#include "sweep_pipe.cuh"
 
 namespace lbm {
 
@@ -10,13 +10,13 @@ int kernel_sets_q21(const KernelSet** out) {
       LBM_KSET(21, double, LBM_RR, false, false),
       LBM_KSET(21, float, LBM_BGK, false, false),
       LBM_KSET(21, float, LBM_RR, false, false),
-      LBM_KSET(21, double, LBM_BGK, true, false),
-      LBM_KSET(21, double, LBM_BGK, true, true),
-      LBM_KSET(21, double, LBM_NUMEQ, false, false),
-      LBM_KSET(21, double, LBM_NUMEQ, true, false),
-      LBM_KSET(21, double, LBM_NUMEQ, true, true),
-      LBM_KSET(21, float, LBM_NUMEQ, true, false),
-      LBM_KSET(21, float, LBM_NUMEQ, true, true)};
+      LBM_KSET_PIPE(21, double, LBM_BGK, true, false),
+      LBM_KSET_PIPE(21, double, LBM_BGK, true, true),
+      LBM_KSET_PIPE(21, double, LBM_NUMEQ, false, false),
+      LBM_KSET_PIPE(21, double, LBM_NUMEQ, true, false),
+      LBM_KSET_PIPE(21, double, LBM_NUMEQ, true, true),
+      LBM_KSET_PIPE(21, float, LBM_NUMEQ, true, false),
+      LBM_KSET_PIPE(21, float, LBM_NUMEQ, true, true)};
   *out = sets;
   return (int)(sizeof(sets) / sizeof(sets[0]));
 }

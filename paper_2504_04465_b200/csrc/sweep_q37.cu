@@ -1,6 +1,6 @@
 // sweep_q37.cu -- D2Q37 instantiations of the level-sweep kernels (sweep.cuh); one translation unit per
 // lattice so that the instantiations compile in parallel.
-#include "sweep.cuh"
+#include "sweep_pipe.cuh"
 
 namespace lbm {
 
@@ -8,12 +8,12 @@ int kernel_sets_q37(const KernelSet** out) {
   static const KernelSet sets[] = {
       LBM_KSET(37, double, LBM_BGK, false, false),
       LBM_KSET(37, double, LBM_RR, false, false),
-      LBM_KSET(37, double, LBM_BGK, true, false),
-      LBM_KSET(37, double, LBM_BGK, true, true),
-      LBM_KSET(37, float, LBM_BGK, true, true),
-      LBM_KSET(37, double, LBM_NUMEQ, true, false),
-      LBM_KSET(37, double, LBM_NUMEQ, true, true),
-      LBM_KSET(37, float, LBM_NUMEQ, true, true)};
+      LBM_KSET_PIPE(37, double, LBM_BGK, true, false),
+      LBM_KSET_PIPE(37, double, LBM_BGK, true, true),
+      LBM_KSET_PIPE(37, float, LBM_BGK, true, true),
+      LBM_KSET_PIPE(37, double, LBM_NUMEQ, true, false),
+      LBM_KSET_PIPE(37, double, LBM_NUMEQ, true, true),
+      LBM_KSET_PIPE(37, float, LBM_NUMEQ, true, true)};
   *out = sets;
   return (int)(sizeof(sets) / sizeof(sets[0]));
 }

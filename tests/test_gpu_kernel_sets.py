@@ -1,7 +1,9 @@
 """Every kernel set the library ships (csrc/sweep_q*.cu, enumerated through lbm_supported_model) has a parity case: a
 two-level periodic stripe (two straight interfaces: coalescence, explosion, fine ghosts, asynchronous schedule) with a
 smooth non-uniform field, two coarse steps, compared with the oracle element by element (f, and g where the model has
-one) at north_star's tolerances; polynomial models in both addressing modes (list and regular bricks)."""
+one) at north_star's tolerances; polynomial models in both addressing modes (list and regular bricks), the wide models
+(second distribution and / or numerical equilibria) also through the software-pipelined sweep with a grid of three CTAs, so
+that every thread walks over several cells."""
 import numpy as np
 import pytest
 
@@ -57,6 +59,14 @@ def test_kernel_set_matches_the_oracle(Q, precision, coll, ddf, sensor):
     for addressing in ((lbm.ADDR_LIST,) if coll == W.NUMEQ else (lbm.ADDR_LIST, lbm.ADDR_BRICKS)):
         g = gpu_from_case(case, precision, addressing=addressing)
         assert ("bricks" in g.kernel_name()) == (addressing == lbm.ADDR_BRICKS)
+        g.step(2)
+        assert g.sync() == 0
+        d = max_pop_diff(g, o, which)
+        assert d <= TOL[precision], (g.kernel_name(), d)
+        g.close()
+    if ddf or coll == W.NUMEQ:
+        g = gpu_from_case(case, precision, pipeline=lbm.PIPE_ALWAYS, pipe_max_ctas=3)
+        assert "sweep_pipe_kernel" in g.kernel_name()
         g.step(2)
         assert g.sync() == 0
         d = max_pop_diff(g, o, which)

@@ -1,0 +1,58 @@
+"""GPU parity of the software-pipelined sweep (csrc/sweep_pipe.cuh; lbm_config.pipeline) on every cell type it handles:
+equilibrium Dirichlet sides with and without density extrapolation, Neumann replicas, bounce-back solids, refinement
+interfaces over several levels (coalescence, explosion, fine ghosts, multiplier warm start), Neumann boxes.  The grid of
+the sweep is capped (lbm_config.pipe_max_ctas) so that a thread walks over many cells with its next cell's gathers in
+flight, and run uncapped on every level (LBM_PIPE_ALWAYS) so that the one-cell-per-thread prologue path is covered too.
+At full size the default mode (LBM_PIPE_AUTO) runs this kernel in tests/test_gpu_fullsize.py."""
+import pytest
+
+from helpers import gpu_from_case, max_pop_diff, oracle_from_case
+from paper_2504_04465_b200 import lbm, workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {64: 1e-12, 32: 1e-5}
+
+CASES = {
+    "naca_subsonic_aoa4": (lambda: W.naca(chord=64, depth=3, radii=(1, 2.5, 5), aoa_deg=4.0), 2, (64,)),
+    "naca_supersonic": (lambda: W.naca(chord=64, depth=2, radii=(1, 2.5), mach=1.5), 2, (64,)),
+    "riemann_q37_poly_neumann_box": (lambda: W.riemann(n=64), 3, (64,)),
+    "riemann_q37_numeq_neumann_box": (lambda: W.riemann(n=48, collision=W.NUMEQ), 2, (64,)),
+    "sod_q21_band": (lambda: W.sod(L=64, lattice=21, mesh="band"), 3, (64, 32)),
+    "sod_q13_sqr": (lambda: W.sod(L=64, lattice=13, mesh="sqr"), 3, (64, 32)),
+    "sod_q37_unif_neumann_ends": (lambda: W.sod(L=64, lattice=37, mesh="unif", periodic=False), 3, (64, 32)),
+}
+
+
+@pytest.mark.parametrize("max_ctas", [0, 1, 5])
+@pytest.mark.parametrize("name", sorted(CASES))
+def test_pipelined_sweep_matches_the_oracle(name, max_ctas):
+    make, ncoarse, precisions = CASES[name]
+    case = make()
+    o = oracle_from_case(case)
+    assert o.step(ncoarse) == 0
+    which = (0, 1, 2) if case.collision == W.NUMEQ else (0, 1)
+    for prec in precisions:
+        g = gpu_from_case(case, prec, pipeline=lbm.PIPE_ALWAYS, pipe_max_ctas=max_ctas)
+        assert "sweep_pipe_kernel" in g.kernel_name()
+        g.step(ncoarse)
+        assert g.sync() == 0
+        d = max_pop_diff(g, o, which[:2])
+        assert d <= TOL[prec], (name, prec, max_ctas, d)
+        if case.collision == W.NUMEQ and prec == 64:
+            # the multipliers are part of the state (Eq. 6-7): they cross the interfaces and warm-start the next solve
+            dl = max_pop_diff(g, o, (2,))
+            assert dl <= 1e-9, (name, dl)
+        g.close()
+
+
+def test_pipelined_and_one_cell_per_thread_sweeps_count_the_same_newton_solves():
+    case = W.naca(chord=64, depth=3, radii=(1, 2.5, 5))
+    counts = []
+    for mode in (lbm.PIPE_OFF, lbm.PIPE_ALWAYS):
+        g = gpu_from_case(case, 64, pipeline=mode, pipe_max_ctas=2)
+        g.step(2)
+        assert g.sync() == 0
+        counts.append(g.newton_iterations())
+        g.close()
+    assert counts[0] == counts[1], counts
