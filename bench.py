@@ -15,6 +15,7 @@ Workloads (synthetic, seeded, shaped like the paper's cases):
   cylinder  BASELINE configs[2]: D2Q9-RR, 6 levels, ~9.85 M cells (default: the multilevel headline)
   uniform   configs[0] scaled to 4096^2 (tree-stored uniform periodic D2Q9-BGK; the 80 %-of-HBM target)
   cavity    configs[1] as given (39 k cells, launch-latency-bound)    cavity8: the same x8
+  cavity:uniform  the paper's uniform lid-driven cavity, L = 4096; with --addressing matrix the Eq. 14 point
   riemann   configs[3]: D2Q37 polynomial + g + sensor, 2048^2        riemann:numeq: the same box with the numerical equilibrium
   naca      configs[4]: D2Q21 numerical equilibrium + g + sensor, 7 levels, ~18 M cells
   sod:<Q>:<mesh>  Table 3 of the paper (numerical equilibrium + g + sensor, single precision there)
@@ -44,10 +45,10 @@ PAPER_TABLE3 = {(13, "unif"): 1259.1, (13, "hori"): 1088.4, (13, "band"): 1244.8
                 (37, "unif"): 286.9, (37, "hori"): 263.0, (37, "band"): 307.4, (37, "sqr"): 266.1}
 REFERENCE_BUDGET_S = 180     # wall-clock cap of the timed region of --impl reference
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only if MEASURED_PEAKS.json is absent
-ADDRESSING = {"auto": 0, "list": 1, "bricks": 2}      # lbm_config.addressing (LBM_ADDR_*)
+ADDRESSING = {"auto": 0, "list": 1, "bricks": 2, "matrix": 3}      # lbm_config.addressing (LBM_ADDR_*)
 PIPELINE = {"auto": 0, "off": 1}                      # lbm_config.pipeline (LBM_PIPE_*): pipelined sweep of the wide models
 # other workloads measured briefly into the default line's `also` (name[@f32|@f64][@list|@bricks])
-DEFAULT_ALSO = "cavity,uniform,cylinder@list,riemann,naca,sod:21:unif@f32"
+DEFAULT_ALSO = "cavity,uniform,uniform@matrix,cylinder@list,riemann,naca,sod:21:unif@f32"
 KERNEL_SOURCES = ("lattice.cuh", "collide.cuh", "sweep.cuh")
 
 
@@ -67,6 +68,9 @@ def make_case(name, scale):
         lat = int(name.split(":")[1])
         return W.tgv(n, lattice=lat, collision=W.RR), dict(
             workload="uniform periodic %dx%d tree-stored D2Q%d-RR Taylor-Green" % (n, n, lat), steps=2000 if lat == 13 else 1200)
+    if name == "cavity:uniform":      # the paper's uniform Cartesian benchmark (Fig. 22): lid-driven cavity, L = 4096
+        n = int(round(4096 * scale))
+        return W.cavity_uniform(n), dict(workload="cavity:uniform (P:520): D2Q9-RR lid-driven cavity on a uniform %dx%d box" % (n, n), steps=4000)
     if name == "cavity":
         return W.cavity(scale), dict(workload="cavity (BASELINE configs[1]): D2Q9-RR, 2 levels, coarse %d^2" % int(128 * scale), steps=100000)
     if name == "cavity8":
@@ -93,6 +97,14 @@ def make_case(name, scale):
     raise SystemExit("unknown workload %r" % name)
 
 
+def label_for(info, addressing):
+    """The workload string of a line; the uniform boxes say which storage they ran in."""
+    w = info["workload"]
+    if addressing == "matrix":
+        w = w.replace("tree-stored", "matrix-like").replace("on a uniform", "on a matrix-like uniform") + " [Cartesian index, AA pattern, one population copy]"
+    return w
+
+
 def npop_of(case):
     return case.lattice * (2 if case.ddf else 1) + (8 if case.collision == W.NUMEQ else 0)
 
@@ -110,6 +122,8 @@ def moved_bytes_per_update(g, case, precision):
     Q = case.lattice
     npop = npop_of(case)
     s = precision // 8
+    if "matrix" in g.kernel_name():        # Cartesian index, AA pattern: the populations once in, once out (Eq. 14 without its 8 B)
+        return float(2 * npop * s)
     bricks = "bricks" in g.kernel_name()
     tot = upd = 0.0
     for l in range(g.depth + 1):
@@ -380,7 +394,7 @@ def also_measure(lbm, entry, precision, dev, peak, peak_src):
     v = upd * steps / (ms * 1e-3) / 1e6
     key = "%s_f%d" % (name, prec) + ("" if opts["addressing"] == "auto" else "@" + opts["addressing"]) + ("" if opts["pipeline"] == "auto" else "@nopipe")
     hbm, alu = roofline_blocks(case, prec, g, key, 1.0, v * 1e6, peak, peak_src, fma_peak_of(lbm, prec) if wants_alu(case) else None)
-    out = {"workload": info["workload"], "entry": entry, "dtype": "f%d" % prec, "value": v, "unit": "MLUPS", "steps": steps,
+    out = {"workload": label_for(info, opts["addressing"]), "entry": entry, "dtype": "f%d" % prec, "value": v, "unit": "MLUPS", "steps": steps,
            "ms_per_step": ms / steps, "cells": g.ntot, "levels": g.depth + 1, "gpu_launches": int(g.info.launches_per_coarse_step) * steps,
            "kernel": g.kernel_name(), "build_s": t_build, "arena_bytes": int(g.info.arena_bytes),
            "mlups_paper_eq13": g.ntot * (1 << g.depth) * steps / (ms * 1e-3) / 1e6}
@@ -523,7 +537,7 @@ def main():
     vs_baseline = None
     if info.get("paper_mlups") and args.precision == 32 and args.scale == 1.0 and world == 1:
         vs_baseline = n_all * (1 << depth) * K / (ms * 1e-3) / 1e6 / info["paper_mlups"]
-    config = workload_config(info, args.precision, depth + 1, n_all, g.n, upd, world)
+    config = workload_config(dict(info, workload=label_for(info, args.addressing)), args.precision, depth + 1, n_all, g.n, upd, world)
     config["l2"] = ("inputs larger than L2 (state %.0f MB)" % (g.info.arena_bytes / 1e6) if g.info.arena_bytes > 4 * 126e6
                     else "working set %.0f MB fits L2: launch-latency-bound case, no flush" % (g.info.arena_bytes / 1e6))
     line = {

@@ -50,7 +50,7 @@ enum { LBM_FLUID = 0, LBM_FINE_GHOST = 1, LBM_COARSE_GHOST = 2, LBM_NEUMANN = 3,
 /* negative link values in the neighbour list */
 enum { LBM_LINK_NONE = -1, LBM_LINK_WALL = -2, LBM_LINK_VBB0 = -3 /* -3-side */ };
 /* device addressing modes (lbm_config.addressing) */
-enum { LBM_ADDR_AUTO = 0, LBM_ADDR_LIST = 1, LBM_ADDR_BRICKS = 2 };
+enum { LBM_ADDR_AUTO = 0, LBM_ADDR_LIST = 1, LBM_ADDR_BRICKS = 2, LBM_ADDR_MATRIX = 3 };
 /* software-pipelined sweep of the wide models (lbm_config.pipeline) */
 enum { LBM_PIPE_AUTO = 0, LBM_PIPE_OFF = 1, LBM_PIPE_ALWAYS = 2 };
 /* error codes */
@@ -85,7 +85,11 @@ typedef struct {
   /* Device-path options (they change how the kernels address memory and how launches are chained, never the result):
    * addressing: LBM_ADDR_AUTO = regular 8x8 bricks by tile arithmetic on levels of >= 2^18 stored cells and the neighbour
    * list elsewhere; LBM_ADDR_LIST = the list-addressed kernel of north_star on every level;
-   * LBM_ADDR_BRICKS = bricks on every level that has some.  no_pdl = 1: plain stream order between level sweeps instead
+   * LBM_ADDR_BRICKS = bricks on every level that has some; LBM_ADDR_MATRIX = the "matrix-like" path of P:512-522 / P:744:
+   * Cartesian-index addressing (no list, no type on the device) with AA-pattern in-place streaming, ONE population copy
+   * (arena_bytes about halves), for single-level boxes (depth 0) without solids or sponge whose sides are periodic,
+   * walls or moving walls, weakly compressible models only -- anything else: LBM_EINVAL.  Host tables and the order of
+   * all host arrays stay the Z-curve storage order.  no_pdl = 1: plain stream order between level sweeps instead
    * of programmatic dependent launch edges.  pipeline: the wide models (second distribution and / or numerical equilibria)
    * run a software-pipelined persistent sweep (gathers of a thread's next cell in flight as cp.async while it computes the
    * current one): LBM_PIPE_AUTO = where it was measured faster (D2Q13 fp32 numerical equilibria), on levels

@@ -12,6 +12,7 @@
 
 #include "../../include/lbm.h"
 #include "grid.hpp"
+#include "matrix.cuh"
 #include "sweep.cuh"
 
 using namespace lbm;
@@ -74,6 +75,9 @@ struct lbm_grid {
   size_t off_tab = 0;
   unsigned short* d_tab = nullptr;
   bool pdl = true;                                // programmatic dependent launch between level sweeps (lbm_config.no_pdl)
+  bool matrix = false;                            // matrix-like uniform path (matrix.cuh): one population copy, no tables on the device
+  size_t off_pos = 0;
+  int* d_pos = nullptr;                           // storage index -> row-major index
   int pf_dist = 0;                                // next-wave L2 prefetch distance of the one-cell-per-thread sweep of the wide models (cells)
   bool pipe = false;                              // software-pipelined persistent sweep on large levels (sweep_pipe.cuh)
   int pipe_grid = 0;                              // resident CTAs of the pipelined sweep on this device (occupancy x SMs)
@@ -130,7 +134,7 @@ const KernelSet* find_kernel_set(const lbm_config& c) {
 
 // n work items, `per_thread` of them per thread.  pdl: chain to the previous kernel of the stream with a programmatic
 // dependent-launch edge (only for kernels that call griddepcontrol.wait before touching mutable data: the sweep).
-int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem = 0, int block = BLOCK);
+int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem = 0, int block = BLOCK, unsigned gridy = 1);
 
 int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s, int per_thread = 1, bool pdl = false, int smem = 0) {
   if (n <= 0) return LBM_OK;
@@ -138,15 +142,15 @@ int launch(const void* fn, int64_t n, void* a0, void* a1, cudaStream_t s, int pe
   return launch_grid(fn, (unsigned)((threads + BLOCK - 1) / BLOCK), a0, a1, s, pdl, smem);
 }
 
-int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem, int block) {
+int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t s, bool pdl, int smem, int block, unsigned gridy) {
   if (grid == 0) return LBM_OK;
   void* args[2] = {a0, a1};
   if (!pdl) {
-    CK(cudaLaunchKernel(fn, dim3(grid), dim3((unsigned)block), args, (size_t)smem, s));
+    CK(cudaLaunchKernel(fn, dim3(grid, gridy), dim3((unsigned)block), args, (size_t)smem, s));
     return LBM_OK;
   }
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = s;
+  cfg.gridDim = dim3(grid, gridy); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = s;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
@@ -155,9 +159,26 @@ int launch_grid(const void* fn, unsigned grid, void* a0, void* a1, cudaStream_t 
   return LBM_OK;
 }
 
+MatrixArgs matrix_args(lbm_grid* g, int parity) {
+  MatrixArgs a = {};
+  a.nx = g->hg.lv[0].nx; a.ny = g->hg.lv[0].ny; a.n = (int)g->dl[0].n;
+  a.ps = g->dl[0].ps; a.A = g->dl[0].S[0]; a.tau = g->hg.lv[0].tau; a.status = g->d_status;
+  a.parity = parity; a.pos = g->d_pos;
+  return a;
+}
+
 // One update of level l (old -> new buffer, coupling with level l-1 fused in), then flip its parity.
 int enqueue_level(lbm_grid* g, int l, int* cur) {
   DevLevel& L = g->dl[l];
+  if (g->matrix) {
+    // matrix-like path: even (layout P0 -> P1) or odd (P1 -> P0) AA step in place, one thread per cell, one grid row per y
+    MatrixArgs ma = matrix_args(g, cur[0]);
+    const int v = (ma.nx % g->ks->matrix_cpt == 0) ? 1 : 0, cpt = v ? g->ks->matrix_cpt : 1;
+    const int rc = launch_grid(g->ks->matrix_step[v][cur[0]], (unsigned)((ma.nx + BLOCK * cpt - 1) / (BLOCK * cpt)), &ma, &g->mp, g->stream,
+                               false, 0, BLOCK, (unsigned)ma.ny);
+    if (rc == LBM_OK) cur[0] ^= 1;
+    return rc;
+  }
   LevelArgs a;
   a.n = (int)L.n; a.ps = L.ps;
   a.So = L.S[cur[l]]; a.Sn = L.S[1 - cur[l]];
@@ -256,7 +277,15 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
   if (cfg->collision < LBM_BGK || cfg->collision > LBM_NUMEQ) return LBM_EINVAL;
   if (cfg->collision == LBM_RR && cfg->ddf) return LBM_EINVAL;     // RR is defined for the athermal models only
   if (!(cfg->tau0 >= 0.5)) return LBM_EINVAL;
-  if (cfg->addressing < LBM_ADDR_AUTO || cfg->addressing > LBM_ADDR_BRICKS) return LBM_EINVAL;
+  if (cfg->addressing < LBM_ADDR_AUTO || cfg->addressing > LBM_ADDR_MATRIX) return LBM_EINVAL;
+  if (cfg->addressing == LBM_ADDR_MATRIX) {
+    // single-level box, weakly compressible, periodic / wall / moving-wall sides, no solids, no sponge
+    if (cfg->depth != 0 || cfg->ddf || cfg->collision == LBM_NUMEQ || cfg->sponge_sigma_max != 0.0) return LBM_EINVAL;
+    if (solid_off && solid_off[1] > solid_off[0]) return LBM_EINVAL;
+    for (int s = 0; s < 4; ++s)
+      if (cfg->bc[s] != LBM_BC_PERIODIC && cfg->bc[s] != LBM_BC_WALL && cfg->bc[s] != LBM_BC_MOVING_WALL && cfg->bc[s] != LBM_BC_INFLOW_VBB)
+        return LBM_EINVAL;
+  }
   if (cfg->pipeline < LBM_PIPE_AUTO || cfg->pipeline > LBM_PIPE_ALWAYS || cfg->pipe_max_ctas < 0) return LBM_EINVAL;
   // the sponge relaxes rho = p / T0: weakly compressible models only
   if (cfg->sponge_sigma_max != 0.0 && (cfg->ddf || cfg->collision == LBM_NUMEQ || !(cfg->sponge_sigma_max > 0.0) ||
@@ -280,7 +309,9 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
     g->depth = cfg->depth;
     g->esize = cfg->precision / 8;
     g->npop = lat.Q * (cfg->ddf ? 2 : 1) + (cfg->collision == LBM_NUMEQ ? LBM_NLAMBDA : 0);
-    g->bricks = ks->sweep_bricks != nullptr && cfg->addressing != LBM_ADDR_LIST;
+    g->matrix = cfg->addressing == LBM_ADDR_MATRIX;
+    if (g->matrix && !ks->matrix_step[0][0]) { delete g; return LBM_EUNSUPPORTED; }
+    g->bricks = ks->sweep_bricks != nullptr && cfg->addressing != LBM_ADDR_LIST && !g->matrix;
     g->brick_min_cells = !g->bricks ? INT64_MAX : cfg->addressing == LBM_ADDR_BRICKS ? 0 : BRICK_MIN_LEVEL_CELLS;
     g->pdl = cfg->no_pdl == 0;
     g->pipe = ks->sweep_pipe != nullptr && (cfg->pipeline == LBM_PIPE_ALWAYS || (cfg->pipeline == LBM_PIPE_AUTO && ks->pipe_auto));
@@ -302,16 +333,23 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
       DevLevel& L = g->dl[l];
       L.n = H.n; L.ng = H.ng;
       L.ps = (int64_t)round_up((size_t)std::max<int64_t>(H.n, 1), 64);   // planes start on 256-byte boundaries
-      L.off_type = off; off += round_up((size_t)L.ps, ALIGN);
-      L.off_aux = off; off += round_up((size_t)L.ps * 4, ALIGN);
-      L.off_nbr = off; off += round_up((size_t)L.ps * 4 * (size_t)(g->Q - 1), ALIGN);
-      L.off_gcoarse = off; off += round_up((size_t)std::max<int64_t>(H.ng, 1) * 4, ALIGN);
-      L.off_gchild = off; off += round_up((size_t)std::max<int64_t>(H.ng, 1) * 16, ALIGN);
-      L.nbrick = H.nbrick; L.n_irr = (int64_t)H.irr.size();
-      L.off_bricks = off; off += round_up((size_t)std::max<int64_t>(H.nbrick, 1) * 36, ALIGN);
-      L.off_irr = off; off += round_up((size_t)std::max<int64_t>(L.n_irr, 1) * 4, ALIGN);
-      L.off_sigma = off; off += round_up(H.sigma.size() * 8, ALIGN);
-      for (int b = 0; b < 2; ++b) { L.off_S[b] = off; off += round_up((size_t)L.ps * (size_t)g->npop * (size_t)g->esize, ALIGN); }
+      if (g->matrix) {
+        // one population copy (AA pattern) and the storage-order map of the I/O kernels; no type, list or ghost tables
+        L.nbrick = 0; L.n_irr = 0;
+        L.off_S[0] = L.off_S[1] = off; off += round_up((size_t)L.ps * (size_t)g->npop * (size_t)g->esize, ALIGN);
+        g->off_pos = off; off += round_up((size_t)L.ps * 4, ALIGN);
+      } else {
+        L.off_type = off; off += round_up((size_t)L.ps, ALIGN);
+        L.off_aux = off; off += round_up((size_t)L.ps * 4, ALIGN);
+        L.off_nbr = off; off += round_up((size_t)L.ps * 4 * (size_t)(g->Q - 1), ALIGN);
+        L.off_gcoarse = off; off += round_up((size_t)std::max<int64_t>(H.ng, 1) * 4, ALIGN);
+        L.off_gchild = off; off += round_up((size_t)std::max<int64_t>(H.ng, 1) * 16, ALIGN);
+        L.nbrick = H.nbrick; L.n_irr = (int64_t)H.irr.size();
+        L.off_bricks = off; off += round_up((size_t)std::max<int64_t>(H.nbrick, 1) * 36, ALIGN);
+        L.off_irr = off; off += round_up((size_t)std::max<int64_t>(L.n_irr, 1) * 4, ALIGN);
+        L.off_sigma = off; off += round_up(H.sigma.size() * 8, ALIGN);
+        for (int b = 0; b < 2; ++b) { L.off_S[b] = off; off += round_up((size_t)L.ps * (size_t)g->npop * (size_t)g->esize, ALIGN); }
+      }
       g->n_total += H.n;
       nmax = std::max(nmax, H.n);
       g->updates_per_coarse += H.n << (g->depth - l);
@@ -445,7 +483,20 @@ int bind_impl(lbm_grid* g, void* dev_arena, void* cuda_stream) {
   CK(cudaMemsetAsync(g->d_status, 0, ALIGN, g->stream));
   const int Q = g->Q;
   std::vector<unsigned char> tbytes;
-  for (int l = 0; l <= g->depth; ++l) {
+  if (g->matrix) {
+    const HostLevel& H = g->hg.lv[0];
+    DevLevel& L = g->dl[0];
+    if (H.ny > 65535) return LBM_EINVAL;            // one grid row per y
+    L.S[0] = L.S[1] = g->arena + L.off_S[0];
+    L.cur = 0;
+    g->d_pos = (int*)(g->arena + g->off_pos);
+    std::vector<int32_t> pos((size_t)H.n);
+    for (int64_t c = 0; c < H.n; ++c) pos[(size_t)c] = H.iy[c] * H.nx + H.ix[c];
+    CK(cudaMemcpyAsync(g->d_pos, pos.data(), (size_t)H.n * 4, cudaMemcpyHostToDevice, g->stream));
+    CK(cudaMemsetAsync(L.S[0], 0, (size_t)L.ps * g->npop * g->esize, g->stream));
+    CK(cudaStreamSynchronize(g->stream));
+  }
+  for (int l = 0; l <= g->depth && !g->matrix; ++l) {
     const HostLevel& H = g->hg.lv[l];
     DevLevel& L = g->dl[l];
     L.type = (unsigned char*)(g->arena + L.off_type);
@@ -477,7 +528,7 @@ int bind_impl(lbm_grid* g, void* dev_arena, void* cuda_stream) {
     for (int b = 0; b < 2; ++b) CK(cudaMemsetAsync(L.S[b], 0, (size_t)L.ps * g->npop * g->esize, g->stream));
   }
   g->d_tab = (unsigned short*)(g->arena + g->off_tab);
-  CK(cudaMemcpyAsync(g->d_tab, g->hg.brick_tab.data(), g->hg.brick_tab.size() * 2, cudaMemcpyHostToDevice, g->stream));
+  if (!g->matrix) CK(cudaMemcpyAsync(g->d_tab, g->hg.brick_tab.data(), g->hg.brick_tab.size() * 2, cudaMemcpyHostToDevice, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   CK(cudaEventCreate(&g->ev0));
   CK(cudaEventCreate(&g->ev1));
@@ -552,6 +603,15 @@ int lbm_init_fields(lbm_grid* g, const double* rho, const double* ux, const doub
   CK(cudaMemcpyAsync(d_ux, ux, N * 8, cudaMemcpyHostToDevice, g->stream));
   CK(cudaMemcpyAsync(d_uy, uy, N * 8, cudaMemcpyHostToDevice, g->stream));
   if (T) CK(cudaMemcpyAsync(d_T, T, N * 8, cudaMemcpyHostToDevice, g->stream));
+  if (g->matrix) {
+    MatrixArgs ma = matrix_args(g, 0);
+    ma.rho = d_rho; ma.ux = d_ux; ma.uy = d_uy;
+    int rc = launch(g->ks->matrix_init, g->dl[0].n, &ma, &g->mp, g->stream);
+    if (rc) return rc;
+    g->dl[0].cur = 0;
+    g->inited = true; g->timed = false; g->kfine = 0;
+    return status_code(g);
+  }
   int64_t base = 0;
   for (int l = 0; l <= g->depth; ++l) {
     DevLevel& L = g->dl[l];
@@ -714,6 +774,7 @@ int lbm_newton_iterations(lbm_grid* g, int64_t* iterations, int64_t* solves) {
 
 const char* lbm_kernel_name(const lbm_grid* g) {
   if (!g) return "";
+  if (g->matrix) return g->ks->matrix_name;
   return (g->pipe && g->hg.lv[0].n >= g->pipe_min_cells) ? g->ks->pipe_name : g->bricks ? g->ks->bricks_name : g->ks->name;
 }
 
@@ -723,8 +784,14 @@ int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double
   DeviceScope dev(g->device);
   const size_t N = (size_t)g->n_total;
   double* d[4] = {g->d_scratch, g->d_scratch + N, g->d_scratch + 2 * N, g->d_scratch + 3 * N};
+  if (g->matrix) {
+    MatrixArgs ma = matrix_args(g, g->dl[0].cur);
+    ma.o_rho = d[0]; ma.o_ux = d[1]; ma.o_uy = d[2]; ma.o_T = d[3];
+    int rc = launch(g->ks->matrix_macro, g->dl[0].n, &ma, &g->mp, g->stream);
+    if (rc) return rc;
+  }
   int64_t base = 0;
-  for (int l = 0; l <= g->depth; ++l) {
+  for (int l = 0; l <= g->depth && !g->matrix; ++l) {
     DevLevel& L = g->dl[l];
     MacroArgs a;
     a.n = (int)L.n; a.ps = L.ps; a.S = L.S[L.cur]; a.cells = nullptr;
@@ -752,10 +819,17 @@ int lbm_get_macroscopic_at(lbm_grid* g, int l, int n, const int32_t* cells, doub
   double* d[4] = {g->d_scratch, g->d_scratch + n, g->d_scratch + 2 * (size_t)n, g->d_scratch + 3 * (size_t)n};
   int* d_cells = (int*)(g->d_scratch + 4 * (size_t)n);
   CK(cudaMemcpyAsync(d_cells, cells, (size_t)n * 4, cudaMemcpyHostToDevice, g->stream));
-  MacroArgs a;
-  a.n = n; a.ps = L.ps; a.S = L.S[L.cur]; a.cells = d_cells;
-  a.rho = d[0]; a.ux = d[1]; a.uy = d[2]; a.Tm = d[3];
-  int rc = launch(g->ks->macro, n, &a, &g->mp, g->stream);
+  int rc;
+  if (g->matrix) {
+    MatrixArgs ma = matrix_args(g, L.cur);
+    ma.n = n; ma.cells = d_cells; ma.o_rho = d[0]; ma.o_ux = d[1]; ma.o_uy = d[2]; ma.o_T = d[3];
+    rc = launch(g->ks->matrix_macro, n, &ma, &g->mp, g->stream);
+  } else {
+    MacroArgs a;
+    a.n = n; a.ps = L.ps; a.S = L.S[L.cur]; a.cells = d_cells;
+    a.rho = d[0]; a.ux = d[1]; a.uy = d[2]; a.Tm = d[3];
+    rc = launch(g->ks->macro, n, &a, &g->mp, g->stream);
+  }
   if (rc) return rc;
   double* h[4] = {rho, ux, uy, T};
   for (int k = 0; k < 4; ++k)
@@ -774,7 +848,12 @@ int lbm_get_populations(lbm_grid* g, int l, int which, double* out) {
   if (L.n == 0) return LBM_OK;
   const long long tot = (long long)L.n * cnt;
   const unsigned grid = (unsigned)((tot + 255) / 256);
-  if (g->esize == 8)
+  if (g->matrix) {
+    MatrixArgs ma = matrix_args(g, L.cur);
+    ma.pops = g->d_scratch;
+    int rc = launch(g->ks->matrix_export, L.n, &ma, &g->mp, g->stream);
+    if (rc) return rc;
+  } else if (g->esize == 8)
     export_kernel<double><<<grid, 256, 0, g->stream>>>((const double*)L.S[L.cur], L.ps, (int)L.n, off, cnt, g->d_scratch);
   else
     export_kernel<float><<<grid, 256, 0, g->stream>>>((const float*)L.S[L.cur], L.ps, (int)L.n, off, cnt, g->d_scratch);
@@ -795,7 +874,12 @@ int lbm_set_populations(lbm_grid* g, int l, int which, const double* in) {
   const long long tot = (long long)L.n * cnt;
   const unsigned grid = (unsigned)((tot + 255) / 256);
   CK(cudaMemcpyAsync(g->d_scratch, in, (size_t)tot * 8, cudaMemcpyHostToDevice, g->stream));
-  if (g->esize == 8)
+  if (g->matrix) {
+    MatrixArgs ma = matrix_args(g, L.cur);
+    ma.pops = g->d_scratch;
+    int rc = launch(g->ks->matrix_import, L.n, &ma, &g->mp, g->stream);
+    if (rc) return rc;
+  } else if (g->esize == 8)
     import_kernel<double><<<grid, 256, 0, g->stream>>>((double*)L.S[L.cur], L.ps, (int)L.n, off, cnt, g->d_scratch);
   else
     import_kernel<float><<<grid, 256, 0, g->stream>>>((float*)L.S[L.cur], L.ps, (int)L.n, off, cnt, g->d_scratch);

@@ -644,6 +644,14 @@ struct KernelSet {
   const char* pipe_name;
   int pipe_tpb, pipe_smem;
   int pipe_auto;            // 1: LBM_PIPE_AUTO selects it on large levels (measured faster than one cell per thread)
+  // matrix-like uniform path (matrix.cuh): even / odd AA step, initialisation, macroscopic, population export / import; or null
+  const void* matrix_step[2][2];      // [one cell per thread | matrix_cpt cells per thread (nx a multiple of it)][even | odd]
+  int matrix_cpt;
+  const void* matrix_init;
+  const void* matrix_macro;
+  const void* matrix_export;
+  const void* matrix_import;
+  const char* matrix_name;
 };
 
 template <int Q, typename T, int COLL, bool DDF, bool SENSOR>
@@ -661,6 +669,7 @@ KernelSet make_kernel_set(const char* name, const char* bricks_name) {
   k.couple = (const void*)&init_coupling_kernel<Q, T, COLL, DDF, SENSOR>;
   k.macro = (const void*)&macroscopic_kernel<Q, T, COLL, DDF>;
   k.sweep_pipe = nullptr; k.pipe_name = ""; k.pipe_tpb = 0; k.pipe_smem = 0; k.pipe_auto = 0;
+  k.matrix_step[0][0] = k.matrix_step[0][1] = k.matrix_step[1][0] = k.matrix_step[1][1] = k.matrix_init = k.matrix_macro = k.matrix_export = k.matrix_import = nullptr; k.matrix_name = ""; k.matrix_cpt = 1;
   return k;
 }
 

@@ -1,15 +1,16 @@
 // sweep_q13.cu -- D2Q13 instantiations of the level-sweep kernels (sweep.cuh); one translation unit per
 // lattice so that the instantiations compile in parallel.
+#include "matrix.cuh"
 #include "sweep_pipe.cuh"
 
 namespace lbm {
 
 int kernel_sets_q13(const KernelSet** out) {
   static const KernelSet sets[] = {
-      LBM_KSET(13, double, LBM_BGK, false, false),
-      LBM_KSET(13, double, LBM_RR, false, false),
-      LBM_KSET(13, float, LBM_BGK, false, false),
-      LBM_KSET(13, float, LBM_RR, false, false),
+      LBM_KSET_MATRIX(13, double, LBM_BGK),
+      LBM_KSET_MATRIX(13, double, LBM_RR),
+      LBM_KSET_MATRIX(13, float, LBM_BGK),
+      LBM_KSET_MATRIX(13, float, LBM_RR),
       LBM_KSET_PIPE(13, double, LBM_BGK, true, false),
       LBM_KSET_PIPE(13, double, LBM_BGK, true, true),
       LBM_KSET_PIPE(13, double, LBM_NUMEQ, false, false),

@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "liblbm_b200.so")
 
 MAX_LEVELS = 24
 BGK, RR, NUMEQ = 0, 1, 2
-ADDR_AUTO, ADDR_LIST, ADDR_BRICKS = 0, 1, 2
+ADDR_AUTO, ADDR_LIST, ADDR_BRICKS, ADDR_MATRIX = 0, 1, 2, 3
 PIPE_AUTO, PIPE_OFF, PIPE_ALWAYS = 0, 1, 2
 BC_PERIODIC, BC_WALL, BC_MOVING_WALL, BC_INFLOW_VBB, BC_DIRICHLET_EQ, BC_DIRICHLET_EQ_RHO_EXTRAP, BC_NEUMANN = range(7)
 FLUID, FINE_GHOST, COARSE_GHOST, NEUMANN, DIRICHLET = range(5)

@@ -159,6 +159,22 @@ def cavity(scale=1.0, collision=RR, re=1000.0, u_lid=0.1, trace_eq=0, lattice=9)
                 meta=dict(N=N, band=band, re=re, u_lid=u_lid, nu0=nu0))
 
 
+def cavity_uniform(n=256, collision=RR, re=1000.0, u_lid=0.1, lattice=9, inflow=0.0):
+    """Lid-driven cavity on a uniform n x n box (the paper's uniform Cartesian benchmark): bounce-back walls, moving
+    lid on top; inflow > 0 adds a wall-normal velocity on the left side (velocity bounce-back with mass flux, tests)."""
+    nu0 = u_lid * n / re
+    tau0 = 0.5 + nu0 / CS2[lattice]
+
+    def fields(level, ix, iy):
+        o = np.ones(len(ix))
+        return o, 0 * o, 0 * o, CS2[lattice] * o
+
+    left = BC_INFLOW_VBB if inflow else BC_WALL
+    return Case("cavity_uniform", uniform_mesh(n, n), lattice=lattice, collision=collision, tau0=tau0,
+                bc=(left, BC_WALL, BC_WALL, BC_MOVING_WALL), bc_ux=(inflow, 0, 0, u_lid), fields=fields,
+                meta=dict(N=n, re=re, u_lid=u_lid, nu0=nu0))
+
+
 # ----------------------------------------------------------------------------- config 3
 CYL_RADII_D = (6.5, 11.0, 17.0, 23.0, 29.0)   # refinement radii R_0..R_4 in cylinder diameters (DESIGN.md)
 

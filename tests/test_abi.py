@@ -171,3 +171,14 @@ def test_compute_calls_fail_loudly_without_device():
     with pytest.raises(lbm.LbmError):
         g.step(1)
     g.close()
+
+
+def test_matrix_addressing_is_refused_where_it_does_not_apply():
+    """LBM_ADDR_MATRIX: single-level boxes without solids, weakly compressible models, periodic / wall sides only."""
+    from paper_2504_04465_b200 import lbm
+    ok = lbm.Grid.from_case(W.tgv(32), addressing=lbm.ADDR_MATRIX)
+    ok.close()
+    for case in (W.cavity(0.25), W.riemann(n=32), W.sod(L=32, lattice=13), W.cylinder(D=40, depth=3, radii=(3, 5, 8))):
+        with pytest.raises(lbm.LbmError) as e:
+            lbm.Grid.from_case(case, addressing=lbm.ADDR_MATRIX)
+        assert e.value.code == lbm.EINVAL

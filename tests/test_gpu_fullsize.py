@@ -36,6 +36,22 @@ def test_uniform_4096_one_step_all_cells():
     assert d[32] <= TOL[32], d
 
 
+def test_uniform_4096_matrix_path_two_steps_all_cells():
+    """bench.py --workload uniform --addressing matrix (the Eq. 14 point): Cartesian index + AA pattern, one even and one
+    odd step, every cell, both precisions."""
+    from paper_2504_04465_b200 import lbm
+    case = W.tgv(4096)
+    o = oracle_from_case(case)
+    assert o.step(2) == 0
+    for prec in (64, 32):
+        g = gpu_from_case(case, prec, addressing=lbm.ADDR_MATRIX)
+        g.step(2)
+        assert g.sync() == 0
+        d = max_pop_diff(g, o, (0,))
+        assert d <= TOL[prec], (prec, d)
+        g.close()
+
+
 def test_cylinder_config3_one_coarse_step_all_cells():
     """bench.py default workload: configs[2], 6 levels, 9.8 M cells, 32 fine steps = 222 M cell updates: every
     interface coalesces and explodes 16..1 times, inflow / Neumann / bounce-back links included."""
