@@ -10,7 +10,7 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRC = ["physics.c", "grid.c", "sim.c"]
+_SRC = ["physics.c", "grid.c", "sim.c", "amr.c"]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 BGK, RR, NUMEQ = 0, 1, 2
@@ -78,6 +78,7 @@ def lib():
         L.orc_get_macroscopic.argtypes = [vp, vp, vp, vp, vp]
         L.orc_get_populations.argtypes = [vp, C.c_int, C.c_int, vp]
         L.orc_set_populations.argtypes = [vp, C.c_int, C.c_int, vp]
+        L.orc_transfer.argtypes = [vp, vp]
         L.orc_lattice.argtypes = [C.c_int, vp, vp, vp, vp, vp, vp]
         L.orc_feq_poly.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, vp]
         L.orc_feq_numerical.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, vp, vp]
@@ -244,6 +245,10 @@ class OracleGrid:
         rc = lib().orc_set_populations(self.h, l, which, _ptr(a))
         if rc != 0:
             raise RuntimeError("orc_set_populations: %d" % rc)
+
+    def transfer_from(self, src):
+        """orc_transfer: takes over the state of `src` (another tree over the same box), Sec. 8.1 of the paper."""
+        return lib().orc_transfer(self.h, src.h)
 
     def newton_iterations(self):
         return int(lib().orc_newton_iterations(self.h))

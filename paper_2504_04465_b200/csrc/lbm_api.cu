@@ -56,6 +56,40 @@ __global__ void import_kernel(T* S, long long ps, int n, int comp0, int cnt, con
   S[(long long)(comp0 + p) * ps + c] = (T)in[(long long)c * cnt + p];
 }
 
+// Re-mesh (lbm_transfer): cell c0 + t of the new level = sum over its plan entries of weight * old state, plane by plane.
+struct TransferArgs {
+  int n, c0, npop;
+  long long ps;
+  void* S;
+  const int* off;                 // [n + 1], relative to ent
+  const lbm::TransferEntry* ent;
+  const void* src[LBM_MAX_LEVELS];
+  long long sps[LBM_MAX_LEVELS];
+};
+
+template <typename T>
+__global__ void __launch_bounds__(128) transfer_kernel(const TransferArgs a) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= a.n) return;
+  const int e0 = a.off[t], e1 = a.off[t + 1];
+  T* S = (T*)a.S;
+  const long long c = (long long)a.c0 + t;
+  if (e1 - e0 == 1 && a.ent[e0].weight == 1.0) {            // copy / uniform explosion: bit for bit
+    const lbm::TransferEntry e = a.ent[e0];
+    const T* src = (const T*)a.src[e.level];
+    for (int q = 0; q < a.npop; ++q) S[q * a.ps + c] = src[q * a.sps[e.level] + e.index];
+    return;
+  }
+  for (int q = 0; q < a.npop; ++q) {                         // coalescence: the weights are 1 / N_f per level crossed
+    double acc = 0.0;
+    for (int k = e0; k < e1; ++k) {
+      const lbm::TransferEntry e = a.ent[k];
+      acc += e.weight * (double)((const T*)a.src[e.level])[q * a.sps[e.level] + e.index];
+    }
+    S[q * a.ps + c] = (T)acc;
+  }
+}
+
 size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 }  // namespace
@@ -723,6 +757,59 @@ int lbm_set_boundary_state(lbm_grid* g, int side, double rho, double ux, double 
   g->hg.cfg.bc_rho[side] = rho; g->hg.cfg.bc_ux[side] = ux; g->hg.cfg.bc_uy[side] = uy; g->hg.cfg.bc_T[side] = T;
   g->mp.bc_rho[side] = rho; g->mp.bc_ux[side] = ux; g->mp.bc_uy[side] = uy; g->mp.bc_T[side] = T;
   drop_graphs(g);
+  return LBM_OK;
+}
+
+int lbm_transfer(lbm_grid* dst, lbm_grid* src) {
+  if (!dst || !src || dst == src) return LBM_EINVAL;
+  if (!dst->bound || !src->bound || !src->inited) return LBM_ESTATE;
+  if (src->kfine != 0) return LBM_ESTATE;
+  if (dst->matrix || src->matrix || dst->device != src->device) return LBM_EINVAL;
+  const lbm_config &a = dst->hg.cfg, &b = src->hg.cfg;
+  if (a.lattice != b.lattice || a.precision != b.precision || a.collision != b.collision || (a.ddf != 0) != (b.ddf != 0)) return LBM_EINVAL;
+  TransferPlan plan;
+  int rc = build_transfer_plan(src->hg, dst->hg, &plan);
+  if (rc) return rc;
+  DeviceScope dev(dst->device);
+  CK(cudaStreamSynchronize(src->stream));
+  dst->inited = false;
+  CK(cudaMemsetAsync(dst->d_status, 0, sizeof(int), dst->stream));
+  TransferArgs ta = {};
+  ta.npop = dst->npop;
+  for (int l = 0; l <= src->depth; ++l) { ta.src[l] = src->dl[l].S[src->dl[l].cur]; ta.sps[l] = src->dl[l].ps; }
+  // the plan goes through dst's scratch area in chunks: [offsets of the chunk | entries of the chunk]
+  const size_t cap = dst->scratch_doubles * 8;
+  std::vector<int32_t> rel;
+  for (int l = 0; l <= dst->depth; ++l) {
+    DevLevel& L = dst->dl[l];
+    const std::vector<int64_t>& off = plan.off[(size_t)l];
+    const std::vector<TransferEntry>& ent = plan.entry[(size_t)l];
+    L.cur = 0;
+    ta.ps = L.ps; ta.S = L.S[0];
+    int64_t c = 0;
+    while (c < L.n) {
+      int64_t c1 = c;
+      while (c1 < L.n && round_up((size_t)(c1 + 1 - c + 1) * 4, 16) + (size_t)(off[(size_t)c1 + 1] - off[(size_t)c]) * sizeof(TransferEntry) <= cap &&
+             c1 - c < (1 << 24))
+        ++c1;
+      if (c1 == c) return LBM_ENOMEM;                       // one cell's entries do not fit the scratch area
+      const int64_t n = c1 - c, ne = off[(size_t)c1] - off[(size_t)c];
+      rel.resize((size_t)n + 1);
+      for (int64_t k = 0; k <= n; ++k) rel[(size_t)k] = (int32_t)(off[(size_t)(c + k)] - off[(size_t)c]);
+      char* base = (char*)dst->d_scratch;
+      const size_t eoff = round_up((size_t)(n + 1) * 4, 16);
+      CK(cudaMemcpyAsync(base, rel.data(), (size_t)(n + 1) * 4, cudaMemcpyHostToDevice, dst->stream));
+      CK(cudaMemcpyAsync(base + eoff, ent.data() + off[(size_t)c], (size_t)ne * sizeof(TransferEntry), cudaMemcpyHostToDevice, dst->stream));
+      ta.n = (int)n; ta.c0 = (int)c; ta.off = (const int*)base; ta.ent = (const TransferEntry*)(base + eoff);
+      const unsigned grid = (unsigned)((n + BLOCK - 1) / BLOCK);
+      if (dst->esize == 8) transfer_kernel<double><<<grid, BLOCK, 0, dst->stream>>>(ta);
+      else transfer_kernel<float><<<grid, BLOCK, 0, dst->stream>>>(ta);
+      CK(cudaGetLastError());
+      CK(cudaStreamSynchronize(dst->stream));              // rel / the chunk of ent are reused by the next chunk
+      c = c1;
+    }
+  }
+  dst->inited = true; dst->timed = false; dst->kfine = 0;
   return LBM_OK;
 }
 

@@ -25,7 +25,7 @@ _ERR = {EINVAL: "LBM_EINVAL", ENOMEM: "LBM_ENOMEM", EMESH: "LBM_EMESH", ECUDA: "
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_supported_model", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
-           "lbm_get_schedule", "lbm_get_sponge", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic", "lbm_get_macroscopic_at",
+           "lbm_get_schedule", "lbm_get_sponge", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_transfer", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic", "lbm_get_macroscopic_at",
            "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_newton_iterations", "lbm_measure_fma_peak"]
 
 
@@ -88,6 +88,7 @@ def lib():
         L.lbm_step_fine.argtypes = [vp, C.c_int]
         L.lbm_set_relaxation.argtypes = [vp, C.c_double]
         L.lbm_set_boundary_state.argtypes = [vp, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double]
+        L.lbm_transfer.argtypes = [vp, vp]
         L.lbm_sync.argtypes = [vp]
         L.lbm_get_macroscopic.argtypes = [vp, vp, vp, vp, vp]
         L.lbm_get_macroscopic_at.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, vp]
@@ -271,6 +272,10 @@ class Grid:
 
     def set_bc_state(self, side, rho, ux, uy, T=0.0):
         _check("lbm_set_boundary_state", lib().lbm_set_boundary_state(self.h, int(side), float(rho), float(ux), float(uy), float(T)))
+
+    def transfer_from(self, src):
+        """lbm_transfer: takes over the state of `src` (another tree over the same box) by copy / explosion / coalescence."""
+        _check("lbm_transfer", lib().lbm_transfer(self.h, src.h))
 
     def sync(self):
         return lib().lbm_sync(self.h)
