@@ -97,6 +97,7 @@ int  orc_get_macroscopic(const orc_grid* g, double* rho, double* ux, double* uy,
 /* which: 0 = f (Q per cell), 1 = g (Q per cell), 2 = lambda (8 per cell); AoS [cell][component] */
 int  orc_get_populations(const orc_grid* g, int level, int which, double* out);
 int  orc_set_populations(orc_grid* g, int level, int which, const double* in);
+int  orc_set_fine_step(orc_grid* g, int64_t k);         /* fine steps taken so far (schedule position), with an imported state */
 /* Mesh adaptation (Sec. 8.1): moves the state of `src` (at a coarse-step boundary) onto `dst`, another tree over the
  * same box with the same model: copy where the old tree stores the cell, uniform explosion from the nearest stored ancestor,
  * else coalescence of the children (amr.c).  dst is then initialised at fine step 0.  ORC_EMESH if dst has a cell the old

@@ -79,6 +79,7 @@ def lib():
         L.orc_get_populations.argtypes = [vp, C.c_int, C.c_int, vp]
         L.orc_set_populations.argtypes = [vp, C.c_int, C.c_int, vp]
         L.orc_transfer.argtypes = [vp, vp]
+        L.orc_set_fine_step.argtypes = [vp, C.c_int64]
         L.orc_lattice.argtypes = [C.c_int, vp, vp, vp, vp, vp, vp]
         L.orc_feq_poly.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, vp]
         L.orc_feq_numerical.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, vp, vp]
@@ -245,6 +246,9 @@ class OracleGrid:
         rc = lib().orc_set_populations(self.h, l, which, _ptr(a))
         if rc != 0:
             raise RuntimeError("orc_set_populations: %d" % rc)
+
+    def set_fine_step(self, k):
+        return lib().orc_set_fine_step(self.h, int(k))
 
     def transfer_from(self, src):
         """orc_transfer: takes over the state of `src` (another tree over the same box), Sec. 8.1 of the paper."""

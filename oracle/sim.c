@@ -406,6 +406,14 @@ static int pop_range(const orc_grid* g, int which, int* off, int* cnt)
   return ORC_EINVAL;
 }
 
+/* position inside the coarse step (fine steps taken since its start), for tests that import a state taken mid-step */
+int orc_set_fine_step(orc_grid* g, int64_t k)
+{
+  if (!g || k < 0) return ORC_EINVAL;
+  g->k = k;
+  return ORC_OK;
+}
+
 int orc_get_populations(const orc_grid* g, int l, int which, double* out)
 {
   int off, cnt;

@@ -140,3 +140,38 @@ def test_naca_config5_sampled_cells_one_fine_step():
     g.step(1)
     assert g.sync() == 0
     g.close()
+
+
+def test_naca_config5_all_levels_all_cells_one_fine_step():
+    """configs[4] at full size, EVERY stored cell of all 7 levels (18.3 M: fluid, coarse and fine ghosts of six interfaces,
+    Dirichlet and Neumann cells, walls of the airfoil): the CUDA path runs 63 fine steps of the schedule, its complete
+    state (f, g, lambda of every level) is handed to the oracle, and both take fine step 64 -- the one in which all levels
+    update, level 0 first: every coalescence (f, g and the multiplier warm start of Eq. 6), collision with the Newton
+    solve, explosion (Eq. 5, 7) and boundary cell of the mesh, in the launch configuration bench.py times."""
+    case = W.naca(chord=1024)
+    g = gpu_from_case(case, 64)
+    nf = 1 << g.depth
+    g.step_fine(nf - 1)
+    assert g.sync() == 0
+    o = oracle_from_case(case, init=False)
+    assert o.n == g.n
+    for l in range(g.depth + 1):
+        for w in (0, 1, 2):
+            o.set_populations(l, w, g.populations(l, w))
+    assert o.set_fine_step(nf - 1) == 0
+    g.step_fine(1)
+    assert g.sync() == 0
+    assert o.step_fine(1) == 0
+    worst = {}
+    for l in range(g.depth + 1):
+        ty = g.cells(l)[2]
+        for w in (0, 1, 2):
+            d = np.abs(g.populations(l, w) - o.populations(l, w)).max(axis=1)
+            for t in np.unique(ty):
+                worst[(w, int(t))] = max(worst.get((w, int(t)), 0.0), float(d[ty == t].max()))
+    assert {t for (_, t) in worst} == {O.FLUID, O.FINE_GHOST, O.COARSE_GHOST, O.NEUMANN, O.DIRICHLET}
+    assert max(v for (w, _), v in worst.items() if w < 2) <= TOL[64], worst
+    assert max(v for (w, _), v in worst.items() if w == 2) <= 1e-9, worst
+    g.step(1)                                   # the schedule is back at a coarse-step boundary: graphs resume
+    assert g.sync() == 0
+    g.close()
