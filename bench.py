@@ -49,7 +49,7 @@ ADDRESSING = {"auto": 0, "list": 1, "bricks": 2, "matrix": 3}      # lbm_config.
 PIPELINE = {"auto": 0, "off": 1}                      # lbm_config.pipeline (LBM_PIPE_*): pipelined sweep of the wide models
 # other workloads measured briefly into the default line's `also` (name[@f32|@f64][@list|@bricks])
 DEFAULT_ALSO = "cavity,uniform,uniform@matrix,cylinder@list,riemann,naca,sod:21:unif@f32"
-KERNEL_SOURCES = ("lattice.cuh", "collide.cuh", "sweep.cuh")
+KERNEL_SOURCES = ("lattice.cuh", "collide.cuh", "sweep.cuh", "sweep_pipe.cuh", "matrix.cuh")
 
 
 def make_case(name, scale):
@@ -430,6 +430,8 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--cpu-baseline-seconds", type=float, default=15.0, help="0 disables the cpu_baseline leg")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--remesh", action="store_true", help="cylinder only: after the timed region, time lbm_transfer onto a tree with "
+                    "other refinement radii (mesh adaptation, Sec. 8.1 of the paper) into the line's `remesh` block")
     ap.add_argument("--also", default=None, help="comma list of other workloads measured briefly into the line's `also` "
                     "(default for the default workload: %s; 'none' disables)" % DEFAULT_ALSO)
     args = ap.parse_args()
@@ -567,6 +569,23 @@ def main():
         line["roofline_alu"] = alu
     if newton:
         line["newton"] = newton
+    if args.remesh and args.workload == "cylinder" and world == 1:
+        # mesh adaptation: the same box with every refinement radius but the outermost moved by one diameter
+        D = int(round(200 * args.scale))
+        t0 = time.perf_counter()
+        case2 = W.cylinder(D=D, radii=tuple(r + (1.0 if k % 2 == 0 else -1.0) for k, r in enumerate(W.CYL_RADII_D[:-1])) + W.CYL_RADII_D[-1:])
+        g2 = lbm.Grid.from_case(case2, precision=args.precision, addressing=ADDRESSING[args.addressing])
+        g2.bind(dev)
+        t1 = time.perf_counter()
+        g2.transfer_from(g)
+        assert g2.sync() == 0
+        t2 = time.perf_counter()
+        g2.step(2)
+        assert g2.sync() == 0
+        line["remesh"] = {"new_tree_build_and_bind_s": t1 - t0, "transfer_s": t2 - t1, "cells_new": g2.ntot, "cells_old": ntot,
+                          "what": "lbm_transfer (host plan: copy / explosion / coalescence per cell of the new tree; device kernel), then two "
+                                  "coarse steps on the new tree ran to status 0; the paper: mesh adaptation on the CPU is the bottleneck (P:698)"}
+        g2.close()
     also = args.also if args.also is not None else (DEFAULT_ALSO if args.workload == "cylinder" and args.scale == 1.0 and args.addressing == "auto" else "none")
     if also != "none" and world == 1:
         g.close()                # release the arena before building the next grid

@@ -100,3 +100,47 @@ def test_byte_accounting_reproduces_the_papers_list_penalty_table():
         assert bench.algorithmic_bytes_per_update(W.tgv(64), prec) == 2 * 9 * s + 8 + 8 * 4 - 4
     naca = W.naca(chord=64, depth=3, radii=(1, 2.5, 5))
     assert bench.algorithmic_bytes_per_update(naca, 64) == 2 * (2 * 21 + 8) * 8 + 8 + 20 * 4 - 4
+
+
+def _bench():
+    import bench
+    return bench
+
+
+def test_roofline_fraction_is_in_moved_bytes_and_flagged_when_implausible():
+    """the headline fraction counts the bytes the kernel moves (a brick cell reads no list), so a kernel at copy
+    speed reads ~1.0, and anything above 1.05 is flagged; the list-addressed figure of SURVEY 8(d) sits beside it."""
+    import types
+    from paper_2504_04465_b200 import workloads as W
+    bench = _bench()
+    case = W.tgv(1024)
+    g = types.SimpleNamespace(depth=0, n=[1024 * 1024], kernel_name=lambda: "sweep_kernel<...> (bricks + list)",
+                              info=types.SimpleNamespace(n_bricks=[1024 * 1024 // 64], brick_min_level_cells=1 << 18))
+    mbpu = bench.moved_bytes_per_update(g, case, 64)
+    assert abs(mbpu - (144 + 36.0 / 64)) < 1e-9
+    peak = 6500.0
+    hbm, alu = bench.roofline_blocks(case, 64, g, "none", 1.0, peak * 1e9 / mbpu, peak, "test", None)
+    assert alu is None and abs(hbm["frac"] - 1.0) < 1e-12 and hbm["frac_plausible"]
+    assert abs(hbm["list_addressed"]["frac"] - 180.0 / mbpu) < 1e-12 and hbm["list_addressed"]["frac"] > 1.2
+    hbm, _ = bench.roofline_blocks(case, 64, g, "none", 1.0, 1.3 * peak * 1e9 / mbpu, peak, "test", None)
+    assert not hbm["frac_plausible"]
+    m = types.SimpleNamespace(depth=0, n=[1024 * 1024], kernel_name=lambda: "matrix_step_kernel<9,double,LBM_BGK> (Cartesian index, AA pattern)",
+                              info=g.info)
+    assert bench.moved_bytes_per_update(m, case, 64) == 144.0
+
+
+def test_committed_bench_lines_have_plausible_fractions():
+    """Every bench line kept under profiles/bench/ for this round: the HBM fraction (moved bytes / measured copy bandwidth) of
+    the headline and of every `also` entry stays <= 1.05."""
+    import glob
+    import json
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "bench", "r02_*.txt")))
+    for f in files:
+        for line in open(f):
+            if not line.startswith("{"):
+                continue
+            d = json.loads(line)
+            for blk in [d] + d.get("also", []):
+                r = blk.get("roofline_hbm") or blk.get("roofline")
+                if r and r.get("bound") == "hbm":
+                    assert r["frac"] <= 1.05, (f, blk.get("entry"), r["frac"])
