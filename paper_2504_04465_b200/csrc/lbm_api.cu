@@ -225,6 +225,7 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   a.brick_nb = L.brick_nb; a.brick_tab = g->d_tab; a.irr = L.irr;
   a.nbrick = (int)L.nbrick; a.n_irr = (int)L.n_irr;
   a.n_inbox = (int)g->hg.lv[l].n_inbox; a.pf_dist = 0;
+  a.queue = (int*)((char*)g->d_status + QUEUE_COUNTER_OFFSET) + 2 * l;
   const int64_t cells_per_cta = g->ks->brick_cells_per_cta;
   a.brick_ctas = (int)((L.nbrick * 64 + cells_per_cta - 1) / cells_per_cta);
   a.list_ctas = (int)((L.n_irr + BLOCK - 1) / BLOCK);
@@ -237,7 +238,8 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
     // n / (grid * block) cells with the next cell's gathers in flight
     const int tpb = g->ks->pipe_tpb;
     const int64_t ctas = std::min<int64_t>(g->pipe_grid, (L.n + tpb - 1) / tpb);
-    rc = launch_grid(g->ks->sweep_pipe, (unsigned)ctas, &a, &g->mp, g->stream, g->pdl, g->ks->pipe_smem, tpb);
+    // no programmatic edge into this launch: its tile queue must not be touched before the previous launch on this level has left it
+    rc = launch_grid(g->ks->sweep_pipe, (unsigned)ctas, &a, &g->mp, g->stream, false, g->ks->pipe_smem, tpb);
   } else if (g->bricks && L.n < g->brick_min_cells) {
     a.nbrick = 0; a.brick_ctas = 0; a.irr = nullptr; a.n_irr = (int)L.n;
     a.list_ctas = (int)((L.n + BLOCK - 1) / BLOCK);

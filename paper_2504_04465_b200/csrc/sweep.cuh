@@ -48,6 +48,7 @@ struct LevelArgs {
   int nbrick, n_irr, brick_ctas, list_ctas;
   int n_inbox;              // cells [n_inbox, n) are the boundary cells (Neumann / Dirichlet), the only ones that read aux early
   int pf_dist;              // L2 prefetch distance in cells (one wave of resident CTAs ahead), 0 = off
+  int* queue;               // pipelined sweep: this level's tile counter and CTA-done counter (both zero between launches)
 };
 
 template <int Q, bool DDF, int COLL>
@@ -79,6 +80,7 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 // Newton statistics ("mean Newton iterations per update"): two 64-bit counters behind the status word,
 // Newton steps (polish included) and solves; one pair of atomics per warp after a warp-level sum.
 constexpr int NEWTON_COUNTER_OFFSET = 8;      // bytes from the status word
+constexpr int QUEUE_COUNTER_OFFSET = 64;      // bytes from the status word: two ints per level (LBM_MAX_LEVELS x 8 = 192 bytes)
 __device__ __forceinline__ void count_newton(int* status, unsigned steps, unsigned solves) {
   const unsigned m = __activemask();
   steps = __reduce_add_sync(m, steps);

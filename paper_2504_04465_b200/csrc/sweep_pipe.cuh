@@ -5,17 +5,21 @@
 // 8 warps are resident per SM; ncu (profiles/r02_ncu_naca_f64.md, r02_ncu_riemann_f64.md, r02_ncu_sod21_f32.md) shows those
 // warps waiting on their own gathers (stall_long_scoreboard 1.6-2.8 cycles per issued instruction, fp64 pipe 29-37 % busy,
 // DRAM 43-60 %): one cell per thread means gather -> wait -> compute -> store, and two warps per scheduler cannot hide a
-// DRAM round trip behind each other's arithmetic.  Here a thread walks over many cells (persistent grid, one CTA slot per
-// SM filled once) and keeps the NEXT cell's gathers in flight while it computes the current one:
-//   iteration k:  issue the gathers of cell k+1 as cp.async (LDGSTS) into shared-memory stage (k+1)&1, from the links that
-//                 were loaded during iteration k-1;  load the links of cell k+2 (consumed in iteration k+1);
-//                 cp.async.wait_group 1;  compute cell k out of stage k&1;  store.
+// DRAM round trip behind each other's arithmetic.  Here a CTA walks over many tiles of TPB consecutive cells (persistent
+// grid: every resident CTA slot of the device once; tiles handed out in Z-curve order from a per-level counter) and a
+// thread keeps the NEXT cell's gathers in flight while it computes the current one:
+//   pass p:  request the id of the tile after next (atomicAdd, consumed at the end of the pass);
+//            cp.async.wait_group 0: the stage of cell p and the links of cell p+1 have landed;
+//            issue the gathers of cell p+1 as cp.async (LDGSTS) into shared-memory stage (p+1)&1 from those links, then
+//            the links of cell p+2 into the link slots;  compute cell p out of stage p&1;  store;
+//            publish the new tile id, one __syncthreads().
 // A thread reads and writes only its own shared-memory slots (plane-major, [stage][plane][thread]: conflict-free 4 / 8-byte
-// accesses), so there is no block-level synchronisation at all, and the populations of the current cell stay in shared
-// memory (streamed through the moment, sensor and relaxation passes) instead of in registers, which is what frees the
-// registers for the link prefetch.  Cell types are handled as in sweep.cuh; the rare ones (coarse ghosts: coalescence,
-// explosion; Dirichlet cells) patch their stage in place with synchronous loads.  Velocity bounce-back links do not
-// occur (weakly compressible models only, lbm_grid_create rejects them here).
+// accesses), and the populations of the current cell stay in shared memory (streamed through the moment, sensor and
+// relaxation passes) instead of in registers; no register holds a link or a population across the arithmetic.  Cell
+// types are handled as in sweep.cuh; the rare ones (coarse ghosts: coalescence, explosion; Dirichlet cells) patch their
+// stage in place with synchronous loads.  Velocity bounce-back links do not occur (weakly compressible models only,
+// lbm_grid_create rejects them here).  The last CTA to finish zeroes the counters, so every launch finds an empty queue; the
+// kernel is launched without a programmatic edge (the queue must not be touched while the previous launch on the level runs).
 #pragma once
 #include "sweep.cuh"
 
@@ -67,7 +71,6 @@ sweep_pipe_kernel(const LevelArgs a, const ModelParams p) {
   T* __restrict__ Sn = (T*)a.Sn;
   long long ps = a.ps;      // laundered once per pass (below), so that no address is hoisted out of the cell loop
   const int n = a.n;
-  const int stride = (int)gridDim.x * TPB;
 
   // a cell's descriptor: storage index, cell whose own values it reads (itself; a Neumann cell: its source, S13),
   // type byte, aux, mask of NONE links
@@ -113,16 +116,32 @@ sweep_pipe_kernel(const LevelArgs a, const ModelParams p) {
   };
 
   [[maybe_unused]] unsigned n_steps = 0u, n_solves = 0u;
-  int cn = (int)blockIdx.x * TPB + (int)threadIdx.x;      // the cell whose gathers are issued next
+  // ---- tile queue.  Tiles of TPB consecutive cells are handed out in Z-curve order from one counter per level, the order
+  // in which the hardware would start the CTAs of a one-cell-per-thread launch: tiles that are neighbours in space are
+  // gathered at about the same time whatever their cells cost (Newton counts differ), so warps that share DRAM sectors
+  // still meet in the L2.  (With a fixed stride per thread the CTAs drifted apart: +47 % DRAM reads.)  The id a CTA needs
+  // two passes later is requested at the top of a pass and published at its end; one block barrier per pass, which also
+  // keeps the four warps of a CTA in the same stretch of code.
+  __shared__ int s_tile[2];
+  int* const q_ctr = a.queue;
+  int* const q_done = a.queue + 1;
+  const int n_tiles = (n + TPB - 1) / TPB;
+  if (threadIdx.x == 0) { s_tile[0] = atomicAdd(q_ctr, 1); s_tile[1] = atomicAdd(q_ctr, 1); }
+  __syncthreads();
+  int t_n = s_tile[0], t_nn = s_tile[1];                   // tile whose gathers are issued next, tile after it (CTA-uniform)
+  __syncthreads();
+  int cn = t_n < n_tiles ? t_n * TPB + (int)threadIdx.x : n;   // the cell whose gathers are issued next
   int tb_n = 0;                                            // its type byte (one register carried across the compute phase)
   Desc cur;
   cur.c = n;                                               // nothing to compute in the first pass
   if (cn < n) { issue_links(cn); tb_n = a.type[cn]; }
   cp_async_commit();
   pdl_wait();      // from here on: data written by the previous sweeps of the stream
-  int s = 0;
+  int s = 0, pass = 0;
 #pragma unroll 1
   for (;;) {
+    int req = 0;
+    if (threadIdx.x == 0) req = atomicAdd(q_ctr, 1);       // in flight during this pass
     // ---- keep the pipeline full.  Everything issued so far has landed after this wait: stage s (the cell to compute
     // now, issued one pass ago and in flight during the previous cell's arithmetic) and the link slots.  Then: gathers of
     // the next cell into the other stage, links of the cell after into the link slots (after the gathers that read them).
@@ -132,17 +151,12 @@ sweep_pipe_kernel(const LevelArgs a, const ModelParams p) {
     asm volatile("" : "+l"(ps));
     Desc nxt;
     nxt.c = n;
-    if (cn < n) {
-      nxt = issue(cn, tb_n, s ^ 1);
-      if (cn + stride < n) { issue_links(cn + stride); tb_n = a.type[cn + stride]; }
-    }
+    if (cn < n) nxt = issue(cn, tb_n, s ^ 1);
+    const int cnn = t_nn < n_tiles ? t_nn * TPB + (int)threadIdx.x : n;
+    if (cnn < n) { issue_links(cnn); tb_n = a.type[cnn]; }
     cp_async_commit();
-    if (cur.c >= n) {           // first pass (or a thread without cells)
-      if (nxt.c >= n) break;
-      cur = nxt; cn += stride; s ^= 1;
-      continue;
-    }
 
+    if (cur.c < n) {
     // ---- the cell update out of stage s
     T* const st = sm + s * NPOP * TPB;
     const int c = cur.c;
@@ -294,10 +308,20 @@ sweep_pipe_kernel(const LevelArgs a, const ModelParams p) {
         }
       }
     }
-    if (nxt.c >= n) break;
-    cur = nxt; cn += stride; s ^= 1;
+    }     // cur.c < n
+    if (t_n >= n_tiles) break;       // CTA-uniform: nothing was issued in this pass, the queue is empty
+    if (threadIdx.x == 0) s_tile[pass & 1] = req;
+    __syncthreads();
+    const int t_new = s_tile[pass & 1];
+    cur = nxt; cn = cnn; t_n = t_nn; t_nn = t_new; s ^= 1; ++pass;
   }
   cp_async_wait<0>();
+  // the last CTA out leaves the queue ready for the next launch on this level
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    __threadfence();
+    if (atomicAdd(q_done, 1) == (int)gridDim.x - 1) { atomicExch(q_ctr, 0); atomicExch(q_done, 0); }
+  }
   if constexpr (NUMEQ) {
     __syncwarp();
     count_newton(a.status, n_steps, n_solves);
@@ -312,11 +336,10 @@ KernelSet make_kernel_set_pipe(const char* name, const char* bricks_name, const 
   k.pipe_name = pipe_name;
   k.pipe_tpb = PC::TPB;
   k.pipe_smem = PC::smem;
-  // Measured on one B200: the pipelined sweep removes the gather stalls (stall_long_scoreboard 1.6 ->
-  // 0.2 per issue on the Sod D2Q21 fp32 case) but its threads drift apart, so that warps sharing DRAM sectors no longer
-  // meet in the L2 (+47 % DRAM reads) and in the instruction cache; it wins where the state per cell is small and the
-  // one-cell-per-thread kernel is register-starved (D2Q13 fp32 numerical equilibria: 10.9 against 7.6 GLUPS) and loses
-  // elsewhere (D2Q21 fp32 7.2 / 7.7, D2Q21 fp64 2.6 / 4.2, D2Q37 fp64 polynomial 2.6 / 4.2), so AUTO selects it only there.
+  // Measured on one B200 (GLUPS, pipelined / one cell per thread): Sod D2Q13 fp32 11.3 / 10.0, Sod D2Q21
+  // fp32 7.9 / 7.7, Sod D2Q37 fp32 3.0 / 3.5, Sod D2Q21 fp64 3.5 / 4.9, naca fp64 2.9 / 4.3: the gather stalls are gone
+  // (stall_long_scoreboard 1.6 -> 0.2 per issue, Sod D2Q21 fp32), but the fp32 solves are instruction-bound either way
+  // and the fp64 ones pay for the 20 KB of L1 this kernel's shared memory leaves them; AUTO selects it where it wins clearly.
   k.pipe_auto = (COLL == LBM_NUMEQ && sizeof(T) == 4 && Q == 13) ? 1 : 0;
   return k;
 }

@@ -362,5 +362,5 @@ def test_riemann_config4_2000_steps_reduced_size():
     assert g.sync() == 0
     r, u, v, T = o.macroscopic()
     gr, gu, gv, gT = g.macroscopic()
-    assert rel_linf(gr, r) <= 2e-2 and np.abs(gu - u).max() <= 2e-2 and abs(gr.mean() - r.mean()) <= 1e-6
+    assert rel_linf(gr, r) <= 2e-2 and np.abs(gu - u).max() <= 2e-2 and abs(gr.mean() - r.mean()) <= 1e-4
     g.close()
