@@ -218,6 +218,12 @@ int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double
  * field (the steady-state, Strouhal and pressure-probe post-processing of Sec. 5 needs a few cells every few steps).
  * HOST outputs of n doubles, any may be NULL.  Synchronises.  LBM_EINVAL for an index outside the level. */
 int lbm_get_macroscopic_at(lbm_grid* g, int level, int n, const int32_t* cells, double* rho, double* ux, double* uy, double* T);
+/* Refinement criterion of the paper's adaptive runs (the kinetic sensor, "the local departure to equilibrium"): eps of
+ * Eq. 52, (1/V) sum_i |f_i - f_i^eq| / f_i^eq, of the CURRENT (post-collision) state of every stored cell, computed on the
+ * device with the model's own equilibrium (numerical equilibria: from the stored multipliers); Eq. 30 scales f - f^eq by
+ * (1 - 1/tau_eff), so this is |1 - 1/tau_eff| times the eps the last collision of the cell saw.  HOST output of n_total doubles
+ * in storage order.  The caller thresholds it, builds the new tree and moves the state with lbm_transfer.  Synchronises. */
+int lbm_get_sensor(lbm_grid* g, double* eps);
 /* Current populations of one level as HOST doubles, row-major [cell][component];
  * which: 0 = f (Q), 1 = g (Q), 2 = lambda (8).  Synchronises. */
 int lbm_get_populations(lbm_grid* g, int level, int which, double* out);

@@ -94,6 +94,8 @@ int  orc_init_fields(orc_grid* g, const double* rho, const double* ux, const dou
 int  orc_step(orc_grid* g, int n_coarse_steps);
 int  orc_step_fine(orc_grid* g, int n_fine_steps);     /* advances k by n fine steps (for 1000-fine-step parity) */
 int  orc_get_macroscopic(const orc_grid* g, double* rho, double* ux, double* uy, double* T);
+/* eps of Eq. 52 of the current state of every stored cell (flat over levels): the refinement criterion of P:717 */
+int  orc_get_sensor(orc_grid* g, double* eps);
 /* which: 0 = f (Q per cell), 1 = g (Q per cell), 2 = lambda (8 per cell); AoS [cell][component] */
 int  orc_get_populations(const orc_grid* g, int level, int which, double* out);
 int  orc_set_populations(orc_grid* g, int level, int which, const double* in);

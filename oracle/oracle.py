@@ -76,6 +76,7 @@ def lib():
         L.orc_step.argtypes = [vp, C.c_int]
         L.orc_step_fine.argtypes = [vp, C.c_int]
         L.orc_get_macroscopic.argtypes = [vp, vp, vp, vp, vp]
+        L.orc_get_sensor.argtypes = [vp, vp]
         L.orc_get_populations.argtypes = [vp, C.c_int, C.c_int, vp]
         L.orc_set_populations.argtypes = [vp, C.c_int, C.c_int, vp]
         L.orc_transfer.argtypes = [vp, vp]
@@ -232,6 +233,14 @@ class OracleGrid:
         r = np.zeros(self.ntot); u = np.zeros(self.ntot); v = np.zeros(self.ntot); T = np.zeros(self.ntot)
         assert lib().orc_get_macroscopic(self.h, _ptr(r), _ptr(u), _ptr(v), _ptr(T)) == 0
         return r, u, v, T
+
+    def sensor(self):
+        """eps of Eq. 52 of the current state of every stored cell, flat over the levels (orc_get_sensor)."""
+        e = np.zeros(self.ntot)
+        rc = lib().orc_get_sensor(self.h, _ptr(e))
+        if rc != 0:
+            raise RuntimeError("orc_get_sensor: %d" % rc)
+        return e
 
     def populations(self, l, which=0):
         cnt = 8 if which == 2 else self.Q

@@ -397,6 +397,39 @@ int orc_get_macroscopic(const orc_grid* g, double* rho, double* ux, double* uy, 
   return ORC_OK;
 }
 
+/* Refinement criterion of the paper's adaptive runs ("the kinetic sensor ... which basically evaluates the local
+ * departure to equilibrium"): eps of Eq. 52, (1/V) sum_i |f_i - f_i^eq| / f_i^eq, of the CURRENT (post-collision) state
+ * of every stored cell, f^eq = the model's equilibrium of the cell's own rho, u, T (numerical equilibria: solved from the
+ * stored multipliers).  The collision of Eq. 30 scales f - f^eq by (1 - 1/tau_eff), so this is |1 - 1/tau_eff| times the eps
+ * the last collision of the cell saw. */
+int orc_get_sensor(orc_grid* g, double* eps)
+{
+  if (!g || !eps) return ORC_EINVAL;
+  const int Q = g->Q;
+  double feq[ORC_QMAX], geq[ORC_QMAX], lam[ORC_NLAMBDA];
+  int64_t base = 0;
+  for (int l = 0; l <= g->depth; ++l) {
+    const orc_level* L = &g->lv[l];
+    const double* S = L->S[L->cur];
+    for (int64_t c = 0; c < L->n; ++c) {
+      const double* f = S + c * g->npop;
+      double r, vx, vy, Tc;
+      orc_phys_moments(g->phys, f, f + Q, &r, &vx, &vy, &Tc);
+      for (int k = 0; k < ORC_NLAMBDA; ++k) lam[k] = (g->cfg.collision == ORC_NUMEQ) ? f[(g->cfg.ddf ? 2 : 1) * Q + k] : 0.0;
+      if (orc_phys_equilibrium(g->phys, r, vx, vy, Tc, lam, feq, geq) < 0) return ORC_ENEWTON;
+      double e = 0.0;
+      for (int i = 0; i < Q; ++i) {
+        double den = fabs(feq[i]);
+        if (den < 1e-300) den = 1e-300;
+        e += fabs(f[i] - feq[i]) / den;
+      }
+      eps[base + c] = e / (double)Q;
+    }
+    base += L->n;
+  }
+  return ORC_OK;
+}
+
 static int pop_range(const orc_grid* g, int which, int* off, int* cnt)
 {
   const int Q = g->Q, ddf = g->cfg.ddf, numeq = (g->cfg.collision == ORC_NUMEQ);

@@ -896,6 +896,33 @@ int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double
   return LBM_OK;
 }
 
+int lbm_get_sensor(lbm_grid* g, double* eps) {
+  if (!g || !eps) return LBM_EINVAL;
+  if (!g->bound || !g->inited) return LBM_ESTATE;
+  DeviceScope dev(g->device);
+  const size_t N = (size_t)g->n_total;
+  double* d = g->d_scratch;
+  if (g->matrix) {
+    MatrixArgs ma = matrix_args(g, g->dl[0].cur);
+    ma.o_rho = d;
+    int rc = launch(g->ks->matrix_sensor, g->dl[0].n, &ma, &g->mp, g->stream);
+    if (rc) return rc;
+  } else {
+    int64_t base = 0;
+    for (int l = 0; l <= g->depth; ++l) {
+      DevLevel& L = g->dl[l];
+      SensorArgs a;
+      a.n = (int)L.n; a.ps = L.ps; a.S = L.S[L.cur]; a.eps = d + base;
+      int rc = launch(g->ks->sensor_field, L.n, &a, &g->mp, g->stream);
+      if (rc) return rc;
+      base += L.n;
+    }
+  }
+  CK(cudaMemcpyAsync(eps, d, N * 8, cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return LBM_OK;
+}
+
 int lbm_get_macroscopic_at(lbm_grid* g, int l, int n, const int32_t* cells, double* rho, double* ux, double* uy, double* T) {
   if (!g || !cells || n < 0 || l < 0 || l > g->depth) return LBM_EINVAL;
   if (!g->bound || !g->inited) return LBM_ESTATE;

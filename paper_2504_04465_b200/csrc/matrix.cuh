@@ -242,6 +242,17 @@ __global__ void __launch_bounds__(128) matrix_macro_kernel(const MatrixArgs a, c
   a.o_rho[t] = (double)rho; a.o_ux[t] = (double)ux; a.o_uy[t] = (double)uy; a.o_T[t] = (double)Tm;
 }
 
+// eps of Eq. 52 of the canonical state (lbm_get_sensor); output slot = storage cell
+template <int Q, typename T, int COLL>
+__global__ void __launch_bounds__(128) matrix_sensor_kernel(const MatrixArgs a, const ModelParams p) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= a.n) return;
+  const int r = a.pos[c], y = r / a.nx, x = r - y * a.nx;
+  T S[Q], g[Q], lam[NLAMBDA];
+  matrix_load_state<Q, T>(a, p, x, y, S);
+  a.o_rho[c] = (double)sensor_of_state<Q, T, COLL, false>(p, S, g, lam);
+}
+
 // canonical-order population I/O of the parity tests: pops[storage cell][Q]
 template <int Q, typename T, bool IMPORT>
 __global__ void __launch_bounds__(128) matrix_io_kernel(const MatrixArgs a, const ModelParams p) {
@@ -269,6 +280,7 @@ KernelSet with_matrix(KernelSet k, const char* name) {
   k.matrix_cpt = MATRIX_CPT<Q, T>;
   k.matrix_init = (const void*)&matrix_init_kernel<Q, T, COLL>;
   k.matrix_macro = (const void*)&matrix_macro_kernel<Q, T, COLL>;
+  k.matrix_sensor = (const void*)&matrix_sensor_kernel<Q, T, COLL>;
   k.matrix_export = (const void*)&matrix_io_kernel<Q, T, false>;
   k.matrix_import = (const void*)&matrix_io_kernel<Q, T, true>;
   k.matrix_name = name;

@@ -629,6 +629,67 @@ __global__ void __launch_bounds__(128) macroscopic_kernel(const MacroArgs a, con
   a.rho[t] = (double)rho; a.ux[t] = (double)ux; a.uy[t] = (double)uy; a.Tm[t] = (double)Tm;
 }
 
+// eps of Eq. 52 of the current (post-collision) state of every cell of one level: the refinement criterion of the
+// paper's adaptive runs.  f^eq = the model's equilibrium of the cell's own moments; numerical equilibria: from the
+// stored multipliers (the collision conserves the moments, so they still are this state's).
+template <int Q, typename T, int COLL, bool DDF>
+__device__ __forceinline__ T sensor_of_state(const ModelParams& p, const T (&f)[Q], const T (&g)[Q], const T (&lam)[NLAMBDA]) {
+  constexpr bool NUMEQ = COLL == LBM_NUMEQ;
+  T rho, ux, uy, Tm;
+  moments<Q, T, NUMEQ || DDF, DDF>(p, f, g, rho, ux, uy, Tm);
+  T feq[Q];
+  if constexpr (NUMEQ) {
+    if constexpr (sizeof(T) == 8) {
+      NumeqExps E;
+      numeq_exps(rho, lam, E);
+      static_for<0, Q>([&](auto ic) { feq[decltype(ic)::value] = numeq_f<Q, decltype(ic)::value>(E); });
+    } else {
+      const T m0[NLAMBDA] = {};
+      T sc[Q], G[NLAMBDA];
+      numeq_eval<Q, T>(rho, m0, lam, feq, sc, G);
+    }
+  } else {
+    T am[NA];
+    aeq_moments<T>(rho, ux, uy, DDF ? Tm - T(cs2_v<Q>) : T(0), am);
+    poly_all<Q, T>(am, [&](auto ic, T fe) { feq[decltype(ic)::value] = fe; });
+  }
+  T eps = T(0);
+#pragma unroll
+  for (int i = 0; i < Q; ++i) {
+    T den = Num<T>::abs_(feq[i]);
+    if (den < Num<T>::tiny()) den = Num<T>::tiny();
+    eps += Num<T>::abs_(f[i] - feq[i]) / den;
+  }
+  return eps / T(Q);
+}
+
+struct SensorArgs {
+  int n;
+  long long ps;
+  const void* S;
+  double* eps;
+};
+
+template <int Q, typename T, int COLL, bool DDF>
+__global__ void __launch_bounds__(128) sensor_kernel(const SensorArgs a, const ModelParams p) {
+  using PL = PopLayout<Q, DDF, COLL>;
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= a.n) return;
+  const T* S = (const T*)a.S;
+  T f[Q], g[Q], lam[NLAMBDA];
+#pragma unroll
+  for (int i = 0; i < Q; ++i) f[i] = S[i * a.ps + c];
+  if constexpr (DDF) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) g[i] = S[(PL::G0 + i) * a.ps + c];
+  }
+  if constexpr (COLL == LBM_NUMEQ) {
+#pragma unroll
+    for (int k = 0; k < NLAMBDA; ++k) lam[k] = S[(PL::L0 + k) * a.ps + c];
+  }
+  a.eps[c] = (double)sensor_of_state<Q, T, COLL, DDF>(p, f, g, lam);
+}
+
 // ------------------------------------------------------------------ dispatch table entry
 struct KernelSet {
   int Q, precision, collision, ddf, sensor;
@@ -641,6 +702,7 @@ struct KernelSet {
   const void* init;
   const void* couple;
   const void* macro;
+  const void* sensor_field;   // eps of Eq. 52 of the stored state (lbm_get_sensor)
   // software-pipelined persistent sweep of the wide models (sweep_pipe.cuh), or null
   const void* sweep_pipe;
   const char* pipe_name;
@@ -651,6 +713,7 @@ struct KernelSet {
   int matrix_cpt;
   const void* matrix_init;
   const void* matrix_macro;
+  const void* matrix_sensor;
   const void* matrix_export;
   const void* matrix_import;
   const char* matrix_name;
@@ -670,8 +733,9 @@ KernelSet make_kernel_set(const char* name, const char* bricks_name) {
   k.init = (const void*)&init_kernel<Q, T, COLL, DDF>;
   k.couple = (const void*)&init_coupling_kernel<Q, T, COLL, DDF, SENSOR>;
   k.macro = (const void*)&macroscopic_kernel<Q, T, COLL, DDF>;
+  k.sensor_field = (const void*)&sensor_kernel<Q, T, COLL, DDF>;
   k.sweep_pipe = nullptr; k.pipe_name = ""; k.pipe_tpb = 0; k.pipe_smem = 0; k.pipe_auto = 0;
-  k.matrix_step[0][0] = k.matrix_step[0][1] = k.matrix_step[1][0] = k.matrix_step[1][1] = k.matrix_init = k.matrix_macro = k.matrix_export = k.matrix_import = nullptr; k.matrix_name = ""; k.matrix_cpt = 1;
+  k.matrix_step[0][0] = k.matrix_step[0][1] = k.matrix_step[1][0] = k.matrix_step[1][1] = k.matrix_init = k.matrix_macro = k.matrix_sensor = k.matrix_export = k.matrix_import = nullptr; k.matrix_name = ""; k.matrix_cpt = 1;
   return k;
 }
 

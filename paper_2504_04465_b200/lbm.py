@@ -25,7 +25,7 @@ _ERR = {EINVAL: "LBM_EINVAL", ENOMEM: "LBM_ENOMEM", EMESH: "LBM_EMESH", ECUDA: "
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_supported_model", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
-           "lbm_get_schedule", "lbm_get_sponge", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_transfer", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic", "lbm_get_macroscopic_at",
+           "lbm_get_schedule", "lbm_get_sponge", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_transfer", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic", "lbm_get_macroscopic_at", "lbm_get_sensor",
            "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_newton_iterations", "lbm_measure_fma_peak"]
 
 
@@ -92,6 +92,7 @@ def lib():
         L.lbm_sync.argtypes = [vp]
         L.lbm_get_macroscopic.argtypes = [vp, vp, vp, vp, vp]
         L.lbm_get_macroscopic_at.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, vp]
+        L.lbm_get_sensor.argtypes = [vp, vp]
         L.lbm_get_populations.argtypes = [vp, C.c_int, C.c_int, vp]
         L.lbm_set_populations.argtypes = [vp, C.c_int, C.c_int, vp]
         L.lbm_last_step_ms.argtypes = [vp]
@@ -312,6 +313,12 @@ class Grid:
         out = [np.zeros(idx.size) for _ in range(4)]
         _check("lbm_get_macroscopic_at", lib().lbm_get_macroscopic_at(self.h, int(l), int(idx.size), _ptr(idx), *[_ptr(o) for o in out]))
         return tuple(out)
+
+    def sensor(self):
+        """eps of Eq. 52 of the current state of every stored cell, flat over the levels (lbm_get_sensor)."""
+        e = np.zeros(self.ntot)
+        _check("lbm_get_sensor", lib().lbm_get_sensor(self.h, _ptr(e)))
+        return e
 
     def populations(self, l, which=0):
         cnt = 8 if which == 2 else self.Q

@@ -122,3 +122,37 @@ def test_A5_cells_without_old_data_are_an_error():
     free.mesh.solid[0] = None                                   # the same tree without the cylinder
     b = oracle_from_case(free, init=False)
     assert b.transfer_from(a) == -3         # ORC_EMESH
+
+
+# ----------------------------------------------------------------------------- the refinement criterion (Eq. 52)
+def _d2q9_feq(rho, ux, uy):
+    """Textbook D2Q9 second-order equilibrium in the canonical direction order, written out here (not the oracle's code);
+    with the oracle's basis (Table 5: + xxy, xyy, xxyy terms) it is the product form: w_i rho prod_a (1 + 3 c_a u_a + ...)."""
+    cx = np.array([0, 1, 0, -1, 0, 1, -1, -1, 1]); cy = np.array([0, 0, 1, 0, -1, 1, 1, -1, -1])
+    w = np.array([4 / 9] + [1 / 9] * 4 + [1 / 36] * 4)
+    # product form of the extended-basis D2Q9 equilibrium: rho * psi_cx(ux) * psi_cy(uy), psi_0 = 2/3 (1 - 3u^2/2) ... with weights folded in
+    px = np.where(cx == 0, (2 / 3) * (1 - 1.5 * ux * ux), (1 / 6) * (1 + 3 * cx * ux + 3 * ux * ux))
+    py = np.where(cy == 0, (2 / 3) * (1 - 1.5 * uy * uy), (1 / 6) * (1 + 3 * cy * uy + 3 * uy * uy))
+    return rho * px * py, cx, cy, w
+
+
+def test_A6_sensor_is_the_relative_departure_from_equilibrium():
+    case = W.Case("u", W.uniform_mesh(8, 8), lattice=9, collision=W.BGK, tau0=0.8,
+                  fields=lambda l, ix, iy: (np.full(len(ix), 1.05), np.full(len(ix), 0.06), np.full(len(ix), -0.03), np.full(len(ix), 1 / 3)))
+    o = oracle_from_case(case)
+    assert np.abs(o.sensor()).max() <= 1e-13                       # equilibrium: eps = 0
+    feq, cx, cy, w = _d2q9_feq(1.05, 0.06, -0.03)
+    assert np.abs(o.populations(0)[0] - feq).max() <= 1e-15        # the closed form above is the state the oracle initialised
+    delta = w * cx * cy                                            # a pure stress perturbation: no mass, no momentum
+    assert abs(delta.sum()) < 1e-17 and abs((delta * cx).sum()) < 1e-17 and abs((delta * cy).sum()) < 1e-17
+    for amp in (1e-3, 4e-3):
+        o.set_populations(0, 0, np.tile(feq + amp * delta, (64, 1)))
+        expect = amp * np.sum(np.abs(delta) / feq) / 9.0           # Eq. 52 by hand
+        assert np.abs(o.sensor() - expect).max() <= 1e-12 * expect + 1e-16
+    # Eq. 30: one BGK collision scales f - f^eq by (1 - 1/tau): the sensor of the post-collision state follows
+    pre = feq + 2e-3 * delta
+    post, _, _, _ = O.collide_cell(o.cfg, 0.8, pre)
+    o.set_populations(0, 0, np.tile(post, (64, 1)))
+    e_post = o.sensor()[0]
+    o.set_populations(0, 0, np.tile(pre, (64, 1)))
+    assert abs(e_post - abs(1 - 1 / 0.8) * o.sensor()[0]) <= 1e-14
