@@ -63,11 +63,11 @@ def make_case(name, scale):
     if name == "uniform":
         n = int(round(4096 * scale))
         return W.tgv(n), dict(workload="uniform periodic %dx%d tree-stored D2Q9-BGK Taylor-Green (configs[0] scaled)" % (n, n), steps=4000)
-    if name in ("uniform:13", "uniform:21"):      # the paper's tree-stored uniform D2Q13-RR / D2Q21-RR points (Fig. 42)
+    if name in ("uniform:13", "uniform:21", "uniform:37"):      # the paper's tree-stored uniform D2Q13-RR / D2Q21-RR points (Fig. 42)
         n = int(round(4096 * scale))
         lat = int(name.split(":")[1])
         return W.tgv(n, lattice=lat, collision=W.RR), dict(
-            workload="uniform periodic %dx%d tree-stored D2Q%d-RR Taylor-Green" % (n, n, lat), steps=2000 if lat == 13 else 1200)
+            workload="uniform periodic %dx%d tree-stored D2Q%d-RR Taylor-Green" % (n, n, lat), steps=2000 if lat == 13 else 1200 if lat == 21 else 600)
     if name == "cavity:uniform":      # the paper's uniform Cartesian benchmark (Fig. 22): lid-driven cavity, L = 4096
         n = int(round(4096 * scale))
         return W.cavity_uniform(n), dict(workload="cavity:uniform (P:520): D2Q9-RR lid-driven cavity on a uniform %dx%d box" % (n, n), steps=4000)
