@@ -425,6 +425,7 @@ def main():
                     "large levels, list = the list-addressed kernel on every level, bricks = bricks on every level")
     ap.add_argument("--pipeline", default="auto", choices=sorted(PIPELINE), help="lbm_config.pipeline: auto = software-pipelined sweep of "
                     "the wide models on large levels, off = one cell per thread everywhere")
+    ap.add_argument("--concurrent-levels", type=int, default=0, choices=[0, 1], help="lbm_config.concurrent_levels (graph branches for levels >= 2, P:221)")
     ap.add_argument("--no-prefetch", type=int, default=0, choices=[0, 1], help="lbm_config.no_prefetch (next-wave L2 prefetch of the wide models)")
     ap.add_argument("--scale", type=float, default=1.0, help="linear scale of the workload (1 = BASELINE size)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
@@ -462,7 +463,7 @@ def main():
 
     t_build = time.perf_counter()
     g = lbm.Grid.from_case(case, precision=args.precision, addressing=ADDRESSING[args.addressing], pipeline=PIPELINE[args.pipeline],
-                           no_prefetch=args.no_prefetch)
+                           no_prefetch=args.no_prefetch, concurrent_levels=args.concurrent_levels)
     g.bind(dev)
     ntot = g.ntot
     pin = lambda: torch.empty(ntot, dtype=torch.float64).pin_memory().numpy()

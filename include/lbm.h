@@ -97,12 +97,16 @@ typedef struct {
    * LBM_PIPE_OFF = never (one cell per thread everywhere), LBM_PIPE_ALWAYS = on every level.  pipe_max_ctas > 0 caps the
    * grid of that sweep (default 0: every resident CTA slot of the device), so that threads walk over more cells.
    * no_prefetch = 1: the one-cell-per-thread sweep of the wide models does not request the next wave's link rows and
-   * population lines into the L2. */
+   * population lines into the L2.  concurrent_levels = 1 (trees of >= 3 levels): in the graphs of
+   * lbm_step the updates of levels >= 2 of a fine step run on a side branch beside the level-0 update of the next fine step
+   * (the overlap proposed; U(0, k+1) depends on U(1, k) only), joined before the next update of level 1; programmatic
+   * dependent launch is then off.  Measured +0.1 % on the six-level cylinder, hence off by default. */
   int addressing;
   int no_pdl;
   int pipeline;
   int pipe_max_ctas;
   int no_prefetch;
+  int concurrent_levels;
 } lbm_config;
 
 typedef struct {

@@ -118,6 +118,12 @@ struct lbm_grid {
   int64_t pipe_min_cells = 0;                     // levels below this keep one cell per thread
   char* arena = nullptr;
   cudaStream_t stream = nullptr;
+  // level-concurrent graphs (lbm_config.concurrent_levels): the updates of levels >= 2 of a fine step are captured on a
+  // side branch beside the level-0 update of the next fine step
+  cudaStream_t launch_stream = nullptr;           // where enqueue_level puts its kernel (stream, or side during a capture)
+  cudaStream_t side = nullptr;
+  cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+  bool concurrent = false;
   int* d_status = nullptr;
   double* d_scratch = nullptr;
   cudaGraphExec_t g1[2] = {nullptr, nullptr};     // one coarse step, starting parity of the coarsest level
@@ -208,7 +214,7 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
     // matrix-like path: even (layout P0 -> P1) or odd (P1 -> P0) AA step in place, one thread per cell, one grid row per y
     MatrixArgs ma = matrix_args(g, cur[0]);
     const int v = (ma.nx % g->ks->matrix_cpt == 0) ? 1 : 0, cpt = v ? g->ks->matrix_cpt : 1;
-    const int rc = launch_grid(g->ks->matrix_step[v][cur[0]], (unsigned)((ma.nx + BLOCK * cpt - 1) / (BLOCK * cpt)), &ma, &g->mp, g->stream,
+    const int rc = launch_grid(g->ks->matrix_step[v][cur[0]], (unsigned)((ma.nx + BLOCK * cpt - 1) / (BLOCK * cpt)), &ma, &g->mp, g->launch_stream,
                                false, 0, BLOCK, (unsigned)ma.ny);
     if (rc == LBM_OK) cur[0] ^= 1;
     return rc;
@@ -239,16 +245,16 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
     const int tpb = g->ks->pipe_tpb;
     const int64_t ctas = std::min<int64_t>(g->pipe_grid, (L.n + tpb - 1) / tpb);
     // no programmatic edge into this launch: its tile queue must not be touched before the previous launch on this level has left it
-    rc = launch_grid(g->ks->sweep_pipe, (unsigned)ctas, &a, &g->mp, g->stream, false, g->ks->pipe_smem, tpb);
+    rc = launch_grid(g->ks->sweep_pipe, (unsigned)ctas, &a, &g->mp, g->launch_stream, false, g->ks->pipe_smem, tpb);
   } else if (g->bricks && L.n < g->brick_min_cells) {
     a.nbrick = 0; a.brick_ctas = 0; a.irr = nullptr; a.n_irr = (int)L.n;
     a.list_ctas = (int)((L.n + BLOCK - 1) / BLOCK);
-    rc = launch_grid(g->ks->sweep_bricks, (unsigned)a.list_ctas, &a, &g->mp, g->stream, g->pdl);
+    rc = launch_grid(g->ks->sweep_bricks, (unsigned)a.list_ctas, &a, &g->mp, g->launch_stream, g->pdl);
   } else if (g->bricks && L.nbrick > 0) {
-    rc = launch_grid(g->ks->sweep_bricks, (unsigned)(a.list_ctas + a.brick_ctas), &a, &g->mp, g->stream, g->pdl);
+    rc = launch_grid(g->ks->sweep_bricks, (unsigned)(a.list_ctas + a.brick_ctas), &a, &g->mp, g->launch_stream, g->pdl);
   } else {
     if (L.n >= 4ll * g->pf_dist) a.pf_dist = g->pf_dist;      // smaller levels live in the L2 anyway
-    rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->stream, g->ks->cells_per_thread, g->pdl);
+    rc = launch(g->ks->sweep, L.n, &a, &g->mp, g->launch_stream, g->ks->cells_per_thread, g->pdl);
   }
   if (rc == LBM_OK) cur[l] ^= 1;
   return rc;
@@ -258,12 +264,31 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
 // level l with k = 0 mod 2^l, ascending.
 int enqueue_coarse_step(lbm_grid* g, int* cur) {
   const int d = g->depth;
-  for (int64_t k = 1; k <= ((int64_t)1 << d); ++k)
+  // Level-concurrent variant (captures only): U(l, k) of fine step k needs U(l-1, k) (its children's values) and hands its
+  // explosion to U(l-1, next), so the chain U(0..L, k) is sequential; but U(0, k+1) needs only U(1, k).  The updates of levels
+  // >= 2 go to a side branch that is joined again before the next update of level 1.
+  const bool conc = g->concurrent && d >= 2;
+  bool forked = false;
+  g->launch_stream = g->stream;
+  for (int64_t k = 1; k <= ((int64_t)1 << d); ++k) {
     for (int l = 0; l <= d; ++l) {
       if (l > 0 && (k % ((int64_t)1 << l)) != 0) break;
+      if (conc && l == 1 && forked) { CK(cudaStreamWaitEvent(g->stream, g->ev_join, 0)); forked = false; }
+      if (conc && l == 2) {
+        CK(cudaEventRecord(g->ev_fork, g->stream));
+        CK(cudaStreamWaitEvent(g->side, g->ev_fork, 0));
+        g->launch_stream = g->side;
+      }
       int rc = enqueue_level(g, l, cur);
-      if (rc) return rc;
+      if (rc) { g->launch_stream = g->stream; return rc; }
     }
+    if (g->launch_stream != g->stream) {
+      CK(cudaEventRecord(g->ev_join, g->side));
+      forked = true;
+      g->launch_stream = g->stream;
+    }
+  }
+  if (forked) CK(cudaStreamWaitEvent(g->stream, g->ev_join, 0));
   return LBM_OK;
 }
 
@@ -349,7 +374,8 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
     if (g->matrix && !ks->matrix_step[0][0]) { delete g; return LBM_EUNSUPPORTED; }
     g->bricks = ks->sweep_bricks != nullptr && cfg->addressing != LBM_ADDR_LIST && !g->matrix;
     g->brick_min_cells = !g->bricks ? INT64_MAX : cfg->addressing == LBM_ADDR_BRICKS ? 0 : BRICK_MIN_LEVEL_CELLS;
-    g->pdl = cfg->no_pdl == 0;
+    g->concurrent = cfg->concurrent_levels != 0 && cfg->depth >= 2;
+    g->pdl = cfg->no_pdl == 0 && !g->concurrent;     // programmatic edges are kept to single-stream chains
     g->pipe = ks->sweep_pipe != nullptr && (cfg->pipeline == LBM_PIPE_ALWAYS || (cfg->pipeline == LBM_PIPE_AUTO && ks->pipe_auto));
     ModelParams& mp = g->mp;
     mp.gamma = cfg->gamma; mp.sensor_A = cfg->sensor_A; mp.T0 = cfg->T0; mp.newton_tol = cfg->newton_tol;
@@ -502,6 +528,9 @@ void release_device_objects(lbm_grid* g) {
   }
   if (g->ev0) { cudaEventDestroy(g->ev0); g->ev0 = nullptr; }
   if (g->ev1) { cudaEventDestroy(g->ev1); g->ev1 = nullptr; }
+  if (g->ev_fork) { cudaEventDestroy(g->ev_fork); g->ev_fork = nullptr; }
+  if (g->ev_join) { cudaEventDestroy(g->ev_join); g->ev_join = nullptr; }
+  if (g->side) { cudaStreamDestroy(g->side); g->side = nullptr; }
   if (g->own_stream && g->stream) cudaStreamDestroy(g->stream);
   g->stream = nullptr; g->own_stream = false;
 }
@@ -568,6 +597,12 @@ int bind_impl(lbm_grid* g, void* dev_arena, void* cuda_stream) {
   CK(cudaStreamSynchronize(g->stream));
   CK(cudaEventCreate(&g->ev0));
   CK(cudaEventCreate(&g->ev1));
+  g->launch_stream = g->stream;
+  if (g->concurrent) {
+    CK(cudaStreamCreateWithFlags(&g->side, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&g->ev_fork, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&g->ev_join, cudaEventDisableTiming));
+  }
   if ((g->hg.cfg.ddf || g->hg.cfg.collision == LBM_NUMEQ) && g->hg.cfg.no_prefetch == 0) {
     // wide models: distance of the next-wave L2 prefetch = the cells one wave of resident CTAs covers
     int per_sm = 0, sms = 0;
@@ -687,6 +722,7 @@ int lbm_step_fine(lbm_grid* g, int n) {
   // uninitialised (every compute call returns LBM_ESTATE until the next lbm_init_fields) instead of running on with
   // buffer parities that no longer describe the device state
   g->inited = false;
+  g->launch_stream = g->stream;
   CK(cudaEventRecord(g->ev0, g->stream));
   for (int s = 0; s < n; ++s) {
     const int64_t k = g->kfine + 1;               // schedule of DESIGN.md Sec. 6 rule 9 at fine step k

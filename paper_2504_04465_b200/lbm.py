@@ -45,7 +45,7 @@ class LbmConfig(C.Structure):
         ("bc_rho", C.c_double * 4), ("bc_ux", C.c_double * 4), ("bc_uy", C.c_double * 4), ("bc_T", C.c_double * 4),
         ("sponge_x0", C.c_double), ("sponge_y0", C.c_double), ("sponge_r0", C.c_double), ("sponge_r1", C.c_double),
         ("sponge_sigma_max", C.c_double), ("sponge_rho_inf", C.c_double),
-        ("addressing", C.c_int), ("no_pdl", C.c_int), ("pipeline", C.c_int), ("pipe_max_ctas", C.c_int), ("no_prefetch", C.c_int),
+        ("addressing", C.c_int), ("no_pdl", C.c_int), ("pipeline", C.c_int), ("pipe_max_ctas", C.c_int), ("no_prefetch", C.c_int), ("concurrent_levels", C.c_int),
     ]
 
 
@@ -133,10 +133,11 @@ def _check(where, rc):
 def make_config(lattice=9, precision=64, collision=BGK, ddf=0, sensor=0, trace_eq=0, depth=0, nx_coarse=1, ny_coarse=1,
                 tau0=0.6, T0=0.0, gamma=1.4, sensor_A=1.5, newton_tol=1e-12, newton_max_iter=50,
                 bc=(0, 0, 0, 0), bc_rho=(1, 1, 1, 1), bc_ux=(0, 0, 0, 0), bc_uy=(0, 0, 0, 0), bc_T=(0, 0, 0, 0),
-                sponge=None, addressing=ADDR_AUTO, no_pdl=0, pipeline=0, pipe_max_ctas=0, no_prefetch=0):
+                sponge=None, addressing=ADDR_AUTO, no_pdl=0, pipeline=0, pipe_max_ctas=0, no_prefetch=0, concurrent_levels=0):
     """sponge: None or (x0, y0, r0, r1, sigma_max, rho_inf) of Eq. 10-11; addressing, no_pdl, pipeline, pipe_max_ctas: device-path options."""
     c = LbmConfig()
     c.addressing, c.no_pdl, c.pipeline, c.pipe_max_ctas, c.no_prefetch = int(addressing), int(no_pdl), int(pipeline), int(pipe_max_ctas), int(no_prefetch)
+    c.concurrent_levels = int(concurrent_levels)
     if sponge is not None:
         (c.sponge_x0, c.sponge_y0, c.sponge_r0, c.sponge_r1, c.sponge_sigma_max, c.sponge_rho_inf) = [float(v) for v in sponge]
     c.lattice, c.precision, c.collision, c.ddf, c.sensor, c.trace_eq = lattice, precision, collision, ddf, sensor, trace_eq

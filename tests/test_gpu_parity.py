@@ -364,3 +364,25 @@ def test_riemann_config4_2000_steps_reduced_size():
     gr, gu, gv, gT = g.macroscopic()
     assert rel_linf(gr, r) <= 2e-2 and np.abs(gu - u).max() <= 2e-2 and abs(gr.mean() - r.mean()) <= 1e-4
     g.close()
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", ["cylinder_small", "naca_small", "patch_depth2"])
+def test_level_concurrent_graphs_match_the_oracle(name):
+    """lbm_config.concurrent_levels (the overlap proposed): the updates of levels >= 2 of a fine step run on a side
+    branch of the captured graph beside the next level-0 update; the result is the same as the sequential schedule's."""
+    case = {"cylinder_small": lambda: W.cylinder(D=40, depth=3, radii=(3, 5, 8)),
+            "naca_small": lambda: W.naca(chord=64, depth=3, radii=(1, 2.5, 5)),
+            "patch_depth2": lambda: W.patch(nc=32, lo=1, hi=31, depth=2, lattice=9, collision=W.RR, tau0=0.7,
+                                            fields=lambda l, ix, iy: (1.0 + 0.03 * np.sin(2 * np.pi * W.centres(l, ix, iy)[0] / 128),
+                                                                      0.05 * np.cos(2 * np.pi * W.centres(l, ix, iy)[1] / 128),
+                                                                      0.02 + 0 * ix, np.full(len(ix), 1 / 3)))}[name]()
+    o = oracle_from_case(case)
+    assert o.step(3) == 0
+    g = gpu_from_case(case, 64, concurrent_levels=1)
+    g.step(1)              # the single-step graph
+    g.step(2)              # both parities of it
+    assert g.sync() == 0
+    d = max_pop_diff(g, o, (0, 1) if case.ddf else (0,))
+    assert d <= 1e-12, (name, d)
+    g.close()
