@@ -56,3 +56,20 @@ def test_pipelined_and_one_cell_per_thread_sweeps_count_the_same_newton_solves()
         counts.append(g.newton_iterations())
         g.close()
     assert counts[0] == counts[1], counts
+
+
+def test_newton_step_count_matches_the_oracles():
+    """"mean Newton iterations per update".  The device counters (lbm_newton_iterations: steps incl. the polish
+    step of S14, over initialisation, iteration-0 coupling, every colliding and Dirichlet cell) against the oracle's own
+    count on the small NACA copy: the same deterministic rule on both sides, so the totals agree up to the few cells whose
+    residual sits within rounding of the tolerance."""
+    case = W.naca(chord=64, depth=3, radii=(1, 2.5, 5), aoa_deg=4.0)
+    o = oracle_from_case(case)
+    g = gpu_from_case(case, 64)
+    assert o.step(2) == 0
+    g.step(2)
+    assert g.sync() == 0
+    steps, solves = g.newton_iterations()
+    assert solves > 0 and abs(steps - o.newton_iterations()) <= 2e-4 * steps, (steps, solves, o.newton_iterations())
+    assert 1.0 <= steps / solves <= 3.0
+    g.close()
