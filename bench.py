@@ -584,7 +584,7 @@ def main():
         g2.step(2)
         assert g2.sync() == 0
         line["remesh"] = {"new_tree_build_and_bind_s": t1 - t0, "transfer_s": t2 - t1, "cells_new": g2.ntot, "cells_old": ntot,
-                          "what": "lbm_transfer (host plan: copy / explosion / coalescence per cell of the new tree; device kernel), then two "
+                          "what": "lbm_transfer (position keys uploaded, look-up + copy / explosion / coalescence per cell of the new tree on the device), then two "
                                   "coarse steps on the new tree ran to status 0; the paper: mesh adaptation on the CPU is the bottleneck (P:698)"}
         g2.close()
     also = args.also if args.also is not None else (DEFAULT_ALSO if args.workload == "cylinder" and args.scale == 1.0 and args.addressing == "auto" else "none")

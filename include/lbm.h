@@ -206,11 +206,12 @@ int lbm_set_boundary_state(lbm_grid* g, int side, double rho, double ux, double 
  * cells included) receives, on the device: the state of the cell src stores at the same level and place (copy); else the
  * state of the nearest stored ancestor (uniform explosion, Eq. 5, 7); else the mean over the children that have data, each
  * by copy or coalescence in turn (Eq. 4, 6: the area-weighted mean of the old cells it covers; children inside solids do
- * not exist); a Neumann cell follows its source cell.  Populations, g and the multipliers lambda alike.  The host builds the
- * plan (lists and weights), a kernel applies it; src's stream is synchronised first, the work runs on dst's stream, and
+ * not exist); a Neumann cell follows its source cell.  Populations, g and the multipliers lambda alike.  The look-up runs on the
+ * device too (binary search in the old tree's position keys, which the storage order keeps sorted); the host only uploads the keys
+ * of the old and the positions of the new tree through the two scratch areas.  src's stream is synchronised first, the work runs on dst's stream, and
  * dst is initialised at fine step 0 afterwards (graphs are captured on its next lbm_step).  src stays valid.
- * LBM_EMESH: dst has a cell where src holds no data (the solids differ); LBM_EINVAL: models, boxes or devices differ, or
- * either grid uses LBM_ADDR_MATRIX; LBM_ESTATE: not bound / not initialised / src inside a coarse step.  Synchronises. */
+ * LBM_EMESH: dst has a cell where src holds no data (the solids differ); LBM_EINVAL: models, boxes or devices differ, either
+ * grid uses LBM_ADDR_MATRIX, or a cell is coarsened over more than three levels at once; LBM_ESTATE: not bound / not initialised / src inside a coarse step.  Synchronises. */
 int lbm_transfer(lbm_grid* dst, lbm_grid* src);
 /* Waits for the stream and returns the sticky device status: LBM_OK, LBM_EUNSTABLE or LBM_ENEWTON. */
 int lbm_sync(lbm_grid* g);

@@ -18,7 +18,7 @@ LIB = os.path.join(HERE, "liblbm_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 
 CU = ["lbm_api.cu", "peak.cu", "sweep_q9.cu", "sweep_q13.cu", "sweep_q21.cu", "sweep_q37.cu"]
-CPP = ["grid_builder.cpp", "transfer.cpp"]
+CPP = ["grid_builder.cpp"]
 HEADERS = sorted(os.path.join(CSRC, h) for h in os.listdir(CSRC) if h.endswith((".cuh", ".hpp", ".h"))) + [os.path.join(INCLUDE, "lbm.h")]
 
 NVCC = os.environ.get("NVCC", "nvcc")

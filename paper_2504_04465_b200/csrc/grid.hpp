@@ -47,16 +47,6 @@ struct HostGrid {
   std::vector<uint16_t> brick_tab;
 };
 
-// Re-mesh plan (transfer.cpp): the state of cell c of level l of the new tree is
-// sum_k weight_k * S_old(level_k, index_k) over entries [off[l][c], off[l][c+1]) -- one entry of weight 1 for a copy or a
-// uniform explosion, the area-weighted old cells below it for a coalescence.
-struct TransferEntry { int32_t index; int32_t level; double weight; };
-struct TransferPlan {
-  std::vector<std::vector<int64_t>> off;
-  std::vector<std::vector<TransferEntry>> entry;
-};
-int build_transfer_plan(const HostGrid& src, const HostGrid& dst, TransferPlan* plan);
-
 // Returns LBM_OK, LBM_EINVAL, LBM_EMESH or LBM_ENOMEM.
 int build_grid(const lbm_config& cfg, const int64_t* split_off, const int32_t* split_xy,
                const int64_t* solid_off, const int32_t* solid_xy, HostGrid* out);

@@ -56,36 +56,129 @@ __global__ void import_kernel(T* S, long long ps, int n, int comp0, int cnt, con
   S[(long long)(comp0 + p) * ps + c] = (T)in[(long long)c * cnt + p];
 }
 
-// Re-mesh (lbm_transfer): cell c0 + t of the new level = sum over its plan entries of weight * old state, plane by plane.
-struct TransferArgs {
-  int n, c0, npop;
+// ---- Re-mesh (lbm_transfer; S25 of DESIGN.md), entirely on the device: every cell of the new tree looks the old
+// tree up by position -- the in-box cells of a level are stored along the Z-curve, so their Morton keys are a sorted array
+// (binary search), the boundary cells are stored by (iy, ix) -- and takes: the cell stored at its own level and place (copy);
+// else the nearest stored ancestor (uniform explosion, Eq. 5, 7); else the mean over the children that have data, each by copy
+// or coalescence in turn (Eq. 4, 6).  A Neumann cell evaluates the rule at its source cell's place.
+constexpr int TR_OFF = 1 << 20;           // boundary layers have negative coordinates
+constexpr int TR_MAX_ENTRIES = 64;        // old cells under one coarsened cell (4^3)
+constexpr int FLAG_EMESH = 4, FLAG_ETOODEEP = 8;
+
+struct TrLevel {
+  const unsigned long long* kin;          // Morton keys of the in-box cells, ascending = storage order
+  const unsigned long long* kb;           // (iy, ix) keys of the boundary cells, ascending = storage order
+  int n_in, n_b, nx, ny;
+  const void* S;
+  long long ps;
+};
+struct TrCtx { TrLevel lv[LBM_MAX_LEVELS]; int depth; };
+struct TrArgs {
+  int n, npop;
   long long ps;
   void* S;
-  const int* off;                 // [n + 1], relative to ent
-  const lbm::TransferEntry* ent;
-  const void* src[LBM_MAX_LEVELS];
-  long long sps[LBM_MAX_LEVELS];
+  const int* ix; const int* iy; const int* aux; const unsigned char* type;
+  int level;
+  int* status;
 };
+struct TrEntry { int index, level; double weight; };
+
+__host__ __device__ inline unsigned long long tr_spread(unsigned v) {
+  unsigned long long x = v;
+  x = (x | (x << 16)) & 0x0000FFFF0000FFFFull;
+  x = (x | (x << 8)) & 0x00FF00FF00FF00FFull;
+  x = (x | (x << 4)) & 0x0F0F0F0F0F0F0F0Full;
+  x = (x | (x << 2)) & 0x3333333333333333ull;
+  x = (x | (x << 1)) & 0x5555555555555555ull;
+  return x;
+}
+__host__ __device__ inline unsigned long long tr_morton(int x, int y) { return tr_spread((unsigned)x) | (tr_spread((unsigned)y) << 1); }
+__host__ __device__ inline unsigned long long tr_bkey(int x, int y) {
+  return ((unsigned long long)(unsigned)(y + TR_OFF) << 32) | (unsigned)(x + TR_OFF);
+}
+
+__device__ int tr_search(const unsigned long long* k, int n, unsigned long long key) {
+  int lo = 0, hi = n - 1;
+  while (lo <= hi) {
+    const int mid = (lo + hi) >> 1;
+    const unsigned long long v = k[mid];
+    if (v == key) return mid;
+    if (v < key) lo = mid + 1; else hi = mid - 1;
+  }
+  return -1;
+}
+
+__device__ int tr_find(const TrCtx& s, int l, int x, int y) {
+  if (l > s.depth) return -1;
+  const TrLevel& L = s.lv[l];
+  if (x >= 0 && y >= 0 && x < L.nx && y < L.ny) return tr_search(L.kin, L.n_in, tr_morton(x, y));
+  const int b = tr_search(L.kb, L.n_b, tr_bkey(x, y));
+  return b < 0 ? -1 : L.n_in + b;
+}
+
+// Coalescence of (l0, x0, y0), a place the old tree does not store: the old cells below it with their weights (1 / N_f per
+// level crossed, N_f = the children that have data), depth first without recursion (a recursive walk would leave the stack
+// size to the device limit).  Invariant: when a node is finished, the entries appended under it carry weights relative to it.
+__device__ bool tr_down(const TrCtx& s, int l0, int x0, int y0, TrEntry* ent, int& n, int* status) {
+  struct Frame { int l, x, y, k, start, nf; };
+  Frame st[4];
+  int d = 0;
+  st[0] = Frame{l0, x0, y0, 0, n, 0};
+  for (;;) {
+    Frame& f = st[d];
+    if (f.l == 0) f.k = 4;                                    // nothing below the finest level
+    if (f.k == 4) {                                           // all children seen
+      const bool found = f.nf > 0;
+      if (found) {
+        for (int e = f.start; e < n; ++e) ent[e].weight = 1.0 * ent[e].weight / (double)f.nf;
+      } else {
+        n = f.start;
+      }
+      if (d == 0) return found;
+      --d;
+      if (found) ++st[d].nf;
+      continue;
+    }
+    const int k = f.k++;
+    const int cl = f.l - 1, cx = 2 * f.x + (k & 1), cy = 2 * f.y + (k >> 1);
+    const int c = tr_find(s, cl, cx, cy);
+    if (c >= 0) {
+      if (n >= TR_MAX_ENTRIES) { atomicOr(status, FLAG_ETOODEEP); return false; }
+      ent[n].index = c; ent[n].level = cl; ent[n].weight = 1.0; ++n;
+      ++f.nf;
+    } else if (cl > 0) {
+      if (d == 3) { atomicOr(status, FLAG_ETOODEEP); return false; }
+      ++d;
+      st[d] = Frame{cl, cx, cy, 0, n, 0};
+    }
+  }
+}
 
 template <typename T>
-__global__ void __launch_bounds__(128) transfer_kernel(const TransferArgs a) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= a.n) return;
-  const int e0 = a.off[t], e1 = a.off[t + 1];
+__global__ void __launch_bounds__(128) transfer_kernel(const TrArgs a, const TrCtx s) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= a.n) return;
+  // a Neumann cell replicates its source cell (S13): it receives what that cell receives
+  const int p = (a.type[c] == LBM_NEUMANN) ? a.aux[c] : c;
+  const int x = a.ix[p], y = a.iy[p], l = a.level;
   T* S = (T*)a.S;
-  const long long c = (long long)a.c0 + t;
-  if (e1 - e0 == 1 && a.ent[e0].weight == 1.0) {            // copy / uniform explosion: bit for bit
-    const lbm::TransferEntry e = a.ent[e0];
-    const T* src = (const T*)a.src[e.level];
-    for (int q = 0; q < a.npop; ++q) S[q * a.ps + c] = src[q * a.sps[e.level] + e.index];
+  int sl = l, sc = tr_find(s, l, x, y);
+  for (int k = 1; sc < 0 && l + k <= s.depth; ++k) {           // nearest stored ancestor (floor division: arithmetic shift)
+    sc = tr_find(s, l + k, x >> k, y >> k);
+    sl = l + k;
+  }
+  if (sc >= 0) {                                                // copy / uniform explosion: bit for bit
+    const T* src = (const T*)s.lv[sl].S;
+    const long long sps = s.lv[sl].ps;
+    for (int q = 0; q < a.npop; ++q) S[q * a.ps + c] = src[q * sps + sc];
     return;
   }
-  for (int q = 0; q < a.npop; ++q) {                         // coalescence: the weights are 1 / N_f per level crossed
+  TrEntry ent[TR_MAX_ENTRIES];
+  int n = 0;
+  if (!tr_down(s, l, x, y, ent, n, a.status)) { atomicOr(a.status, FLAG_EMESH); return; }
+  for (int q = 0; q < a.npop; ++q) {                            // coalescence: weights 1 / N_f per level crossed
     double acc = 0.0;
-    for (int k = e0; k < e1; ++k) {
-      const lbm::TransferEntry e = a.ent[k];
-      acc += e.weight * (double)((const T*)a.src[e.level])[q * a.sps[e.level] + e.index];
-    }
+    for (int k = 0; k < n; ++k) acc += ent[k].weight * (double)((const T*)s.lv[ent[k].level].S)[q * s.lv[ent[k].level].ps + ent[k].index];
     S[q * a.ps + c] = (T)acc;
   }
 }
@@ -805,47 +898,83 @@ int lbm_transfer(lbm_grid* dst, lbm_grid* src) {
   if (dst->matrix || src->matrix || dst->device != src->device) return LBM_EINVAL;
   const lbm_config &a = dst->hg.cfg, &b = src->hg.cfg;
   if (a.lattice != b.lattice || a.precision != b.precision || a.collision != b.collision || (a.ddf != 0) != (b.ddf != 0)) return LBM_EINVAL;
-  TransferPlan plan;
-  int rc = build_transfer_plan(src->hg, dst->hg, &plan);
-  if (rc) return rc;
+  if (src->hg.lat.Q != dst->hg.lat.Q) return LBM_EINVAL;
+  if (((int64_t)b.nx_coarse << src->depth) != ((int64_t)a.nx_coarse << dst->depth) ||
+      ((int64_t)b.ny_coarse << src->depth) != ((int64_t)a.ny_coarse << dst->depth))
+    return LBM_EINVAL;
   DeviceScope dev(dst->device);
   CK(cudaStreamSynchronize(src->stream));
   dst->inited = false;
   CK(cudaMemsetAsync(dst->d_status, 0, sizeof(int), dst->stream));
-  TransferArgs ta = {};
-  ta.npop = dst->npop;
-  for (int l = 0; l <= src->depth; ++l) { ta.src[l] = src->dl[l].S[src->dl[l].cur]; ta.sps[l] = src->dl[l].ps; }
-  // the plan goes through dst's scratch area in chunks: [offsets of the chunk | entries of the chunk]
-  const size_t cap = dst->scratch_doubles * 8;
-  std::vector<int32_t> rel;
-  for (int l = 0; l <= dst->depth; ++l) {
-    DevLevel& L = dst->dl[l];
-    const std::vector<int64_t>& off = plan.off[(size_t)l];
-    const std::vector<TransferEntry>& ent = plan.entry[(size_t)l];
-    L.cur = 0;
-    ta.ps = L.ps; ta.S = L.S[0];
-    int64_t c = 0;
-    while (c < L.n) {
-      int64_t c1 = c;
-      while (c1 < L.n && round_up((size_t)(c1 + 1 - c + 1) * 4, 16) + (size_t)(off[(size_t)c1 + 1] - off[(size_t)c]) * sizeof(TransferEntry) <= cap &&
-             c1 - c < (1 << 24))
-        ++c1;
-      if (c1 == c) return LBM_ENOMEM;                       // one cell's entries do not fit the scratch area
-      const int64_t n = c1 - c, ne = off[(size_t)c1] - off[(size_t)c];
-      rel.resize((size_t)n + 1);
-      for (int64_t k = 0; k <= n; ++k) rel[(size_t)k] = (int32_t)(off[(size_t)(c + k)] - off[(size_t)c]);
-      char* base = (char*)dst->d_scratch;
-      const size_t eoff = round_up((size_t)(n + 1) * 4, 16);
-      CK(cudaMemcpyAsync(base, rel.data(), (size_t)(n + 1) * 4, cudaMemcpyHostToDevice, dst->stream));
-      CK(cudaMemcpyAsync(base + eoff, ent.data() + off[(size_t)c], (size_t)ne * sizeof(TransferEntry), cudaMemcpyHostToDevice, dst->stream));
-      ta.n = (int)n; ta.c0 = (int)c; ta.off = (const int*)base; ta.ent = (const TransferEntry*)(base + eoff);
-      const unsigned grid = (unsigned)((n + BLOCK - 1) / BLOCK);
-      if (dst->esize == 8) transfer_kernel<double><<<grid, BLOCK, 0, dst->stream>>>(ta);
-      else transfer_kernel<float><<<grid, BLOCK, 0, dst->stream>>>(ta);
-      CK(cudaGetLastError());
-      CK(cudaStreamSynchronize(dst->stream));              // rel / the chunk of ent are reused by the next chunk
-      c = c1;
+  // position keys of the old tree -> src's scratch area (8 bytes per cell), level after level
+  TrCtx ctx = {};
+  ctx.depth = src->depth;
+  {
+    std::vector<unsigned long long> keys((size_t)src->n_total);
+    size_t base = 0;
+    for (int l = 0; l <= src->depth; ++l) {
+      const HostLevel& H = src->hg.lv[l];
+      for (int64_t c = 0; c < H.n; ++c)
+        keys[base + (size_t)c] = c < H.n_inbox ? tr_morton(H.ix[c], H.iy[c]) : tr_bkey(H.ix[c], H.iy[c]);
+      for (int64_t c = 1; c < H.n; ++c)       // the storage order IS the key order (DESIGN.md Sec. 6 rule 6): what the search relies on
+        if (c != H.n_inbox && keys[base + (size_t)c] <= keys[base + (size_t)c - 1]) return LBM_EINVAL;
+      TrLevel& L = ctx.lv[l];
+      L.kin = (const unsigned long long*)src->d_scratch + base;
+      L.kb = L.kin + H.n_inbox;
+      L.n_in = (int)H.n_inbox; L.n_b = (int)(H.n - H.n_inbox); L.nx = H.nx; L.ny = H.ny;
+      L.S = src->dl[l].S[src->dl[l].cur]; L.ps = src->dl[l].ps;
+      base += (size_t)H.n;
     }
+    if (keys.size() > src->scratch_doubles) return LBM_ENOMEM;
+    CK(cudaMemcpyAsync(src->d_scratch, keys.data(), keys.size() * 8, cudaMemcpyHostToDevice, dst->stream));
+    CK(cudaStreamSynchronize(dst->stream));
+  }
+  // positions, types and sources of the new tree -> dst's scratch area (13 bytes per cell), then one launch per level
+  {
+    const size_t N = (size_t)dst->n_total;
+    if (4 * N * 4 > dst->scratch_doubles * 8) return LBM_ENOMEM;
+    std::vector<int32_t> hix(N), hiy(N), haux(N);
+    std::vector<unsigned char> hty(N);
+    size_t base = 0;
+    for (int l = 0; l <= dst->depth; ++l) {
+      const HostLevel& H = dst->hg.lv[l];
+      for (int64_t c = 0; c < H.n; ++c) {
+        hix[base + (size_t)c] = H.ix[c]; hiy[base + (size_t)c] = H.iy[c]; haux[base + (size_t)c] = H.aux[c];
+        hty[base + (size_t)c] = H.type[c];
+        if (H.type[c] == LBM_NEUMANN && (H.aux[c] < 0 || H.aux[c] >= H.n)) return LBM_EMESH;
+      }
+      base += (size_t)H.n;
+    }
+    int* d_ix = (int*)dst->d_scratch;
+    int* d_iy = d_ix + N;
+    int* d_aux = d_iy + N;
+    unsigned char* d_ty = (unsigned char*)(d_aux + N);
+    CK(cudaMemcpyAsync(d_ix, hix.data(), N * 4, cudaMemcpyHostToDevice, dst->stream));
+    CK(cudaMemcpyAsync(d_iy, hiy.data(), N * 4, cudaMemcpyHostToDevice, dst->stream));
+    CK(cudaMemcpyAsync(d_aux, haux.data(), N * 4, cudaMemcpyHostToDevice, dst->stream));
+    CK(cudaMemcpyAsync(d_ty, hty.data(), N, cudaMemcpyHostToDevice, dst->stream));
+    base = 0;
+    for (int l = 0; l <= dst->depth; ++l) {
+      DevLevel& L = dst->dl[l];
+      L.cur = 0;
+      TrArgs ta = {};
+      ta.n = (int)L.n; ta.npop = dst->npop; ta.ps = L.ps; ta.S = L.S[0];
+      ta.ix = d_ix + base; ta.iy = d_iy + base; ta.aux = d_aux + base; ta.type = d_ty + base;
+      ta.level = l; ta.status = dst->d_status;
+      const unsigned grid = (unsigned)((L.n + BLOCK - 1) / BLOCK);
+      if (grid > 0) {
+        if (dst->esize == 8) transfer_kernel<double><<<grid, BLOCK, 0, dst->stream>>>(ta, ctx);
+        else transfer_kernel<float><<<grid, BLOCK, 0, dst->stream>>>(ta, ctx);
+        CK(cudaGetLastError());
+      }
+      base += (size_t)L.n;
+    }
+    int flags = 0;
+    CK(cudaMemcpyAsync(&flags, dst->d_status, sizeof(int), cudaMemcpyDeviceToHost, dst->stream));
+    CK(cudaStreamSynchronize(dst->stream));                    // the host vectors above live until here
+    CK(cudaMemsetAsync(dst->d_status, 0, sizeof(int), dst->stream));
+    if (flags & FLAG_EMESH) return LBM_EMESH;                 // the old tree has no data under a cell of the new one
+    if (flags & FLAG_ETOODEEP) return LBM_EINVAL;             // a cell coarsened over more than three levels at once
   }
   dst->inited = true; dst->timed = false; dst->kfine = 0;
   return LBM_OK;

@@ -1,4 +1,4 @@
-"""GPU parity of lbm_transfer (mesh adaptation, Sec. 8.1 of the paper P:696-698; csrc/transfer.cpp + transfer_kernel)
+"""GPU parity of lbm_transfer (mesh adaptation, Sec. 8.1 of the paper P:696-698; transfer_kernel of csrc/lbm_api.cu: look-up and transfer on the device)
 against the oracle's orc_transfer on the same pairs of trees: a refined patch that moves and deepens (copy, explosion,
 coalescence over one and two levels, ghost bands on both sides), the graded cylinder mesh with other radii (solid cells:
 N_f < 4, inflow / Neumann boundary cells), the NACA mesh with numerical equilibria (g and the multipliers lambda move too,
