@@ -573,6 +573,9 @@ def main():
     if args.remesh and args.workload == "cylinder" and world == 1:
         # mesh adaptation: the same box with every refinement radius but the outermost moved by one diameter
         D = int(round(200 * args.scale))
+        tc = time.perf_counter()
+        eps = g.sensor()                 # the refinement criterion (Eq. 52 of the stored state), computed on the device
+        tc = time.perf_counter() - tc
         t0 = time.perf_counter()
         case2 = W.cylinder(D=D, radii=tuple(r + (1.0 if k % 2 == 0 else -1.0) for k, r in enumerate(W.CYL_RADII_D[:-1])) + W.CYL_RADII_D[-1:])
         g2 = lbm.Grid.from_case(case2, precision=args.precision, addressing=ADDRESSING[args.addressing])
@@ -583,7 +586,7 @@ def main():
         t2 = time.perf_counter()
         g2.step(2)
         assert g2.sync() == 0
-        line["remesh"] = {"new_tree_build_and_bind_s": t1 - t0, "transfer_s": t2 - t1, "cells_new": g2.ntot, "cells_old": ntot,
+        line["remesh"] = {"criterion_s": tc, "criterion_max": float(eps.max()), "new_tree_build_and_bind_s": t1 - t0, "transfer_s": t2 - t1, "cells_new": g2.ntot, "cells_old": ntot,
                           "what": "lbm_transfer (position keys uploaded, look-up + copy / explosion / coalescence per cell of the new tree on the device), then two "
                                   "coarse steps on the new tree ran to status 0; the paper: mesh adaptation on the CPU is the bottleneck (P:698)"}
         g2.close()
