@@ -22,6 +22,8 @@ namespace {
 constexpr int BLOCK = 128;
 constexpr int64_t BRICK_MIN_LEVEL_CELLS = 1 << 18;
 constexpr size_t ALIGN = 256;
+static_assert(lbm::QUEUE_COUNTER_OFFSET + 8 * LBM_MAX_LEVELS <= (int)ALIGN && lbm::NEWTON_COUNTER_OFFSET + 16 <= lbm::QUEUE_COUNTER_OFFSET,
+              "status word, Newton counters and the tile queues of all levels share the first ALIGN bytes of the arena");
 
 struct DevLevel {
   int64_t n = 0, ps = 0, ng = 0;
