@@ -48,7 +48,7 @@ FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md, used only 
 ADDRESSING = {"auto": 0, "list": 1, "bricks": 2, "matrix": 3}      # lbm_config.addressing (LBM_ADDR_*)
 PIPELINE = {"auto": 0, "off": 1, "always": 2}                    # lbm_config.pipeline (LBM_PIPE_*): pipelined sweep of the wide models
 # other workloads measured briefly into the default line's `also` (name[@f32|@f64][@list|@bricks])
-DEFAULT_ALSO = "cavity,uniform,uniform@matrix,cylinder@list,riemann,naca,sod:21:unif@f32"
+DEFAULT_ALSO = "cavity,uniform,uniform@matrix,uniform@matrix@f32,cylinder@list,cylinder@f32,riemann,naca,sod:21:unif@f32"
 KERNEL_SOURCES = ("lattice.cuh", "collide.cuh", "sweep.cuh", "sweep_pipe.cuh", "matrix.cuh")
 
 
