@@ -887,9 +887,28 @@ int lbm_set_relaxation(lbm_grid* g, double tau0) {
 
 int lbm_set_boundary_state(lbm_grid* g, int side, double rho, double ux, double uy, double T) {
   if (!g || side < 0 || side > 3) return LBM_EINVAL;
+  // matrix-like path: Ladd's term of the OLD wall velocity is folded into the stored wall slots (matrix.cuh); the state is taken
+  // out with the old parameters and put back with the new ones, so that the next pull sees the new wall velocity as the list
+  // path (and the oracle) would
+  const bool rebake = g->matrix && g->bound && g->inited;
+  if (rebake) {
+    DeviceScope dev(g->device);
+    MatrixArgs ma = matrix_args(g, g->dl[0].cur);
+    ma.pops = g->d_scratch;
+    int rc = launch(g->ks->matrix_export, g->dl[0].n, &ma, &g->mp, g->stream);
+    if (rc) return rc;
+    CK(cudaStreamSynchronize(g->stream));          // the kernel read g->mp by value at launch; be explicit all the same
+  }
   g->hg.cfg.bc_rho[side] = rho; g->hg.cfg.bc_ux[side] = ux; g->hg.cfg.bc_uy[side] = uy; g->hg.cfg.bc_T[side] = T;
   g->mp.bc_rho[side] = rho; g->mp.bc_ux[side] = ux; g->mp.bc_uy[side] = uy; g->mp.bc_T[side] = T;
   drop_graphs(g);
+  if (rebake) {
+    DeviceScope dev(g->device);
+    MatrixArgs ma = matrix_args(g, g->dl[0].cur);
+    ma.pops = g->d_scratch;
+    int rc = launch(g->ks->matrix_import, g->dl[0].n, &ma, &g->mp, g->stream);
+    if (rc) return rc;
+  }
   return LBM_OK;
 }
 

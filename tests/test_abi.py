@@ -182,3 +182,13 @@ def test_matrix_addressing_is_refused_where_it_does_not_apply():
         with pytest.raises(lbm.LbmError) as e:
             lbm.Grid.from_case(case, addressing=lbm.ADDR_MATRIX)
         assert e.value.code == lbm.EINVAL
+
+
+def test_device_options_are_validated():
+    """lbm_config.addressing / pipeline / pipe_max_ctas outside their ranges: LBM_EINVAL, no grid."""
+    from paper_2504_04465_b200 import lbm
+    case = W.tgv(16)
+    for bad in (dict(addressing=7), dict(addressing=-1), dict(pipeline=3), dict(pipe_max_ctas=-2)):
+        with pytest.raises(lbm.LbmError) as e:
+            lbm.Grid.from_case(case, **bad)
+        assert e.value.code == lbm.EINVAL

@@ -131,3 +131,28 @@ def test_matrix_arena_is_one_population_copy_and_no_tables():
     assert m.info.arena_bytes < 0.62 * t.info.arena_bytes
     assert m.info.arena_bytes <= n * (9 * 8 + 4 + 9 * 8) + 4096      # populations + order map + I/O scratch
     m.close(); t.close()
+
+
+def test_matrix_path_follows_the_viscosity_and_lid_ramps_and_refuses_transfer():
+    """lbm_set_relaxation / lbm_set_boundary_state between steps (the start-up ramps) on the matrix-like path against
+    the oracle's setters, with single fine steps in between; lbm_transfer does not apply to it."""
+    case = W.cavity_uniform(72)
+    o = oracle_from_case(case)
+    g = gpu_from_case(case, 64, addressing=lbm.ADDR_MATRIX)
+    tau0 = case.tau0
+    for step in range(6):
+        t = W.viscosity_ramp_tau0(tau0, step, 5, factor=20.0)
+        lid = 0.1 * W.mach_ramp_factor(step, 5)
+        g.set_tau0(t); assert o.set_tau0(t) == 0
+        g.set_bc_state(3, 1.0, lid, 0.0); assert o.set_bc_state(3, 1.0, lid, 0.0) == 0
+        if step % 2:
+            g.step_fine(3); assert o.step_fine(3) == 0
+        else:
+            g.step(2); assert o.step(2) == 0
+        assert g.sync() == 0
+    assert max_pop_diff(g, o) <= 4e-12
+    other = gpu_from_case(W.cavity_uniform(72), 64, init=False)
+    with pytest.raises(lbm.LbmError) as e:
+        other.transfer_from(g)
+    assert e.value.code == lbm.EINVAL
+    g.close(); other.close()
