@@ -255,10 +255,12 @@ def test_viscosity_and_lid_velocity_ramp_cavity():
     g.close()
 
 
-def test_mach_ramp_on_dirichlet_sides_naca():
-    """Numerical-equilibrium Dirichlet sides driven through the Mach ramp of P:424."""
+@pytest.mark.parametrize("options", [{}, dict(pipeline=2, pipe_max_ctas=4), dict(concurrent_levels=1)], ids=["default", "pipelined", "concurrent"])
+def test_mach_ramp_on_dirichlet_sides_naca(options):
+    """Numerical-equilibrium Dirichlet sides driven through the Mach ramp of P:424; also through the pipelined sweep and
+    the level-concurrent graphs (the graphs are re-captured after every change of the boundary state)."""
     case = W.naca(chord=64, depth=3, radii=(1, 2.5, 5))
-    g = gpu_from_case(case, 64)
+    g = gpu_from_case(case, 64, **options)
     o = oracle_from_case(case)
     for step in range(4):
         m = W.mach_ramp_factor(step, 3, start=0.8)
