@@ -38,6 +38,7 @@ extern "C" {
 #define LBM_MAX_LEVELS 24
 #define LBM_QMAX 37
 #define LBM_NLAMBDA 8
+#define LBM_STATIC_PROBE_MAX 4096   /* probe cells per lbm_get_macroscopic_at_static call (144 KB of static device memory) */
 
 /* collision models: BGK with polynomial equilibrium (Eq. 30, 34), recursive regularised (Eq. 33-38),
  * BGK with numerical equilibrium (Eq. 39-49) */
@@ -58,7 +59,8 @@ enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_EMESH = -3, LBM_ECUDA =
        LBM_EUNSTABLE = -5 /* non-finite or non-positive density */,
        LBM_ENEWTON = -6 /* Newton-Raphson did not converge */,
        LBM_EUNSUPPORTED = -7 /* model combination has no compiled kernel */,
-       LBM_ESTATE = -8 /* call order: not bound / not initialised */ };
+       LBM_ESTATE = -8 /* call order: not bound / not initialised */,
+       LBM_ETOOLARGE = -9 /* request beyond a fixed capacity (lbm_get_macroscopic_at_static: LBM_STATIC_PROBE_MAX) */ };
 
 typedef struct {
   int lattice;        /* 9, 13, 21, 37 (Table 4) */
@@ -223,6 +225,16 @@ int lbm_get_macroscopic(lbm_grid* g, double* rho, double* ux, double* uy, double
  * field (the steady-state, Strouhal and pressure-probe post-processing of Sec. 5 needs a few cells every few steps).
  * HOST outputs of n doubles, any may be NULL.  Synchronises.  LBM_EINVAL for an index outside the level. */
 int lbm_get_macroscopic_at(lbm_grid* g, int level, int n, const int32_t* cells, double* rho, double* ux, double* uy, double* T);
+/* lbm_get_macroscopic_at without any scratch from the caller and without any allocation: same arguments, same results
+ * (the same kernel), but the staging area (the cell indices and the four output arrays on the device) is a file-scope
+ * `static __device__` array of the library, LBM_STATIC_PROBE_MAX cells = 144 KB, which every GPU that loads the library
+ * holds until the process exits.  For callers that may not allocate (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc) and do not want the library to touch the scratch part of their arena.  The call makes no
+ * cudaMalloc / cudaFree and calls no allocating routine.  n > LBM_STATIC_PROBE_MAX: LBM_ETOOLARGE, nothing is done (use
+ * lbm_get_macroscopic_at).  ALL grids of the process on one GPU share the one array and it keeps the last call's contents
+ * (nothing in it needs to start at zero: every slot read is written first by the same call); two calls that overlap on the
+ * GPU -- different grids on different streams, or two host threads -- race on it: serialise them.  Synchronises. */
+int lbm_get_macroscopic_at_static(lbm_grid* g, int level, int n, const int32_t* cells, double* rho, double* ux, double* uy, double* T);
 /* Refinement criterion of the paper's adaptive runs (the kinetic sensor, "the local departure to equilibrium"): eps of
  * Eq. 52, (1/V) sum_i |f_i - f_i^eq| / f_i^eq, of the CURRENT (post-collision) state of every stored cell, computed on the
  * device with the model's own equilibrium (numerical equilibria: from the stored multipliers); Eq. 30 scales f - f^eq by

@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1122,6 +1123,72 @@ int lbm_get_macroscopic_at(lbm_grid* g, int l, int n, const int32_t* cells, doub
   int* d_cells = (int*)(g->d_scratch + 4 * (size_t)n);
   CK(cudaMemcpyAsync(d_cells, cells, (size_t)n * 4, cudaMemcpyHostToDevice, g->stream));
   int rc;
+  if (g->matrix) {
+    MatrixArgs ma = matrix_args(g, L.cur);
+    ma.n = n; ma.cells = d_cells; ma.o_rho = d[0]; ma.o_ux = d[1]; ma.o_uy = d[2]; ma.o_T = d[3];
+    rc = launch(g->ks->matrix_macro, n, &ma, &g->mp, g->stream);
+  } else {
+    MacroArgs a;
+    a.n = n; a.ps = L.ps; a.S = L.S[L.cur]; a.cells = d_cells;
+    a.rho = d[0]; a.ux = d[1]; a.uy = d[2]; a.Tm = d[3];
+    rc = launch(g->ks->macro, n, &a, &g->mp, g->stream);
+  }
+  if (rc) return rc;
+  double* h[4] = {rho, ux, uy, T};
+  for (int k = 0; k < 4; ++k)
+    if (h[k]) CK(cudaMemcpyAsync(h[k], d[k], (size_t)n * 8, cudaMemcpyDeviceToHost, g->stream));
+  CK(cudaStreamSynchronize(g->stream));
+  return LBM_OK;
+}
+
+}  // extern "C"
+
+// ---- lbm_get_macroscopic_at_static: the probe-cell read-out with its scratch in a file-scope device array instead of the
+// caller's arena (for callers that hand the library no scratch area and may not allocate: include/lbm.h).  Layout of the
+// array: [cells: MAX int32 | rho | ux | uy | T: MAX doubles each].  Every GPU that loads the library holds it until exit.
+namespace {
+constexpr int STATIC_PROBE_MAX = LBM_STATIC_PROBE_MAX;
+constexpr size_t STATIC_PROBE_BYTES = (size_t)STATIC_PROBE_MAX * (4 + 4 * 8);
+static __device__ __align__(256) unsigned char g_static_probe_scratch[STATIC_PROBE_BYTES];
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_probe_mutex;
+void* g_static_probe_addr[STATIC_MAX_DEVICES] = {};     // device address of the array per device ordinal (0 = not asked yet)
+
+// In host code the array's name is a host-side stand-in, not a device address: the address comes from cudaGetSymbolAddress,
+// once per device, with that device current (the caller holds a DeviceScope).
+int static_probe_scratch(int device, unsigned char** out) {
+  if (device < 0 || device >= STATIC_MAX_DEVICES) return LBM_EINVAL;
+  std::lock_guard<std::mutex> lock(g_static_probe_mutex);
+  if (!g_static_probe_addr[device]) {
+    void* ptr = nullptr;
+    if (cudaGetSymbolAddress(&ptr, g_static_probe_scratch) != cudaSuccess || !ptr) { cudaGetLastError(); return LBM_ECUDA; }
+    g_static_probe_addr[device] = ptr;
+  }
+  *out = (unsigned char*)g_static_probe_addr[device];
+  return LBM_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int lbm_get_macroscopic_at_static(lbm_grid* g, int l, int n, const int32_t* cells, double* rho, double* ux, double* uy, double* T) {
+  if (!g || !cells || n < 0 || l < 0 || l > g->depth) return LBM_EINVAL;
+  if (n > STATIC_PROBE_MAX) return LBM_ETOOLARGE;           // beyond the static scratch: use lbm_get_macroscopic_at
+  if (!g->bound || !g->inited) return LBM_ESTATE;
+  if (n == 0) return LBM_OK;
+  DeviceScope dev(g->device);
+  DevLevel& L = g->dl[l];
+  for (int k = 0; k < n; ++k)
+    if (cells[k] < 0 || cells[k] >= L.n) return LBM_EINVAL;
+  unsigned char* base = nullptr;
+  int rc = static_probe_scratch(g->device, &base);
+  if (rc) return rc;
+  int* d_cells = (int*)base;
+  double* d0 = (double*)(base + (size_t)STATIC_PROBE_MAX * 4);
+  double* d[4] = {d0, d0 + STATIC_PROBE_MAX, d0 + 2 * (size_t)STATIC_PROBE_MAX, d0 + 3 * (size_t)STATIC_PROBE_MAX};
+  // the array keeps the previous call's contents; nothing in it has to start at zero: the n index slots are overwritten by
+  // this copy and the 4 n output slots by the kernel before anything reads them, and only those are copied back
+  CK(cudaMemcpyAsync(d_cells, cells, (size_t)n * 4, cudaMemcpyHostToDevice, g->stream));
   if (g->matrix) {
     MatrixArgs ma = matrix_args(g, L.cur);
     ma.n = n; ma.cells = d_cells; ma.o_rho = d[0]; ma.o_ux = d[1]; ma.o_uy = d[2]; ma.o_T = d[3];

@@ -19,13 +19,14 @@ PIPE_AUTO, PIPE_OFF, PIPE_ALWAYS = 0, 1, 2
 BC_PERIODIC, BC_WALL, BC_MOVING_WALL, BC_INFLOW_VBB, BC_DIRICHLET_EQ, BC_DIRICHLET_EQ_RHO_EXTRAP, BC_NEUMANN = range(7)
 FLUID, FINE_GHOST, COARSE_GHOST, NEUMANN, DIRICHLET = range(5)
 LINK_NONE, LINK_WALL, LINK_VBB0 = -1, -2, -3
-OK, EINVAL, ENOMEM, EMESH, ECUDA, EUNSTABLE, ENEWTON, EUNSUPPORTED, ESTATE = 0, -1, -2, -3, -4, -5, -6, -7, -8
+OK, EINVAL, ENOMEM, EMESH, ECUDA, EUNSTABLE, ENEWTON, EUNSUPPORTED, ESTATE, ETOOLARGE = 0, -1, -2, -3, -4, -5, -6, -7, -8, -9
+STATIC_PROBE_MAX = 4096
 _ERR = {EINVAL: "LBM_EINVAL", ENOMEM: "LBM_ENOMEM", EMESH: "LBM_EMESH", ECUDA: "LBM_ECUDA", EUNSTABLE: "LBM_EUNSTABLE",
-        ENEWTON: "LBM_ENEWTON", EUNSUPPORTED: "LBM_EUNSUPPORTED", ESTATE: "LBM_ESTATE"}
+        ENEWTON: "LBM_ENEWTON", EUNSUPPORTED: "LBM_EUNSUPPORTED", ESTATE: "LBM_ESTATE", ETOOLARGE: "LBM_ETOOLARGE"}
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["lbm_grid_create", "lbm_destroy", "lbm_grid_query", "lbm_supported_model", "lbm_get_cells", "lbm_get_nbr", "lbm_get_ghosts",
-           "lbm_get_schedule", "lbm_get_sponge", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_transfer", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic", "lbm_get_macroscopic_at", "lbm_get_sensor",
+           "lbm_get_schedule", "lbm_get_sponge", "lbm_get_bricks", "lbm_grid_bind", "lbm_init_fields", "lbm_step", "lbm_step_fine", "lbm_transfer", "lbm_set_relaxation", "lbm_set_boundary_state", "lbm_sync", "lbm_get_macroscopic", "lbm_get_macroscopic_at", "lbm_get_macroscopic_at_static", "lbm_get_sensor",
            "lbm_get_populations", "lbm_set_populations", "lbm_last_step_ms", "lbm_kernel_name", "lbm_newton_iterations", "lbm_measure_fma_peak"]
 
 
@@ -92,6 +93,7 @@ def lib():
         L.lbm_sync.argtypes = [vp]
         L.lbm_get_macroscopic.argtypes = [vp, vp, vp, vp, vp]
         L.lbm_get_macroscopic_at.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, vp]
+        L.lbm_get_macroscopic_at_static.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, vp]
         L.lbm_get_sensor.argtypes = [vp, vp]
         L.lbm_get_populations.argtypes = [vp, C.c_int, C.c_int, vp]
         L.lbm_set_populations.argtypes = [vp, C.c_int, C.c_int, vp]
@@ -320,6 +322,15 @@ class Grid:
         e = np.zeros(self.ntot)
         _check("lbm_get_sensor", lib().lbm_get_sensor(self.h, _ptr(e)))
         return e
+
+    def macroscopic_at_static(self, l, cells):
+        """The same through lbm_get_macroscopic_at_static: scratch in the library's static device array, no allocation,
+        at most STATIC_PROBE_MAX cells per call."""
+        idx = np.ascontiguousarray(cells, dtype=np.int32)
+        out = [np.zeros(idx.size) for _ in range(4)]
+        _check("lbm_get_macroscopic_at_static",
+               lib().lbm_get_macroscopic_at_static(self.h, int(l), int(idx.size), _ptr(idx), *[_ptr(o) for o in out]))
+        return tuple(out)
 
     def populations(self, l, which=0):
         cnt = 8 if which == 2 else self.Q
