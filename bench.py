@@ -14,6 +14,7 @@ shard: DESIGN.md "replicas only"), no data-path collective; value = sum over ran
 Workloads (synthetic, seeded, shaped like the paper's cases):
   cylinder  BASELINE configs[2]: D2Q9-RR, 6 levels, ~9.85 M cells (default: the multilevel headline)
   uniform   configs[0] scaled to 4096^2 (tree-stored uniform periodic D2Q9-BGK; the 80 %-of-HBM target)
+  cylinder:mc<k> / cylinder:mf<k>  the same box with k levels merged from the coarsest / finest (the paper's Table 2 study)
   cavity    configs[1] as given (39 k cells, launch-latency-bound)    cavity8: the same x8
   cavity:uniform  the paper's uniform lid-driven cavity, L = 4096; with --addressing matrix the Eq. 14 point
   riemann   configs[3]: D2Q37 polynomial + g + sensor, 2048^2        riemann:numeq: the same box with the numerical equilibrium
@@ -56,6 +57,17 @@ def make_case(name, scale):
     if name == "cylinder":
         D = int(round(200 * scale))
         return W.cylinder(D=D), dict(workload="cylinder (BASELINE configs[2]): D2Q9-RR, D=%d, 64Dx64D, 6 levels" % D, steps=300)
+    if name.startswith("cylinder:mc") or name.startswith("cylinder:mf"):
+        # the paper's grid-hierarchy study (Sec. 7.5, Table 2, Fig. 24) at fixed finest resolution: levels merged from
+        # the coarsest (mc<k>: the k+1 coarsest levels become one) or from the finest (mf<k>: the k+1 finest levels become
+        # level 0); k = 5 is the uniform finest grid either way
+        k = int(name[11:])
+        D = int(round(200 * scale))
+        coarse = name[10] == "c"
+        radii = W.CYL_RADII_D[:5 - k] if coarse else W.CYL_RADII_D[k:]
+        return W.cylinder(D=D, depth=5 - k, radii=radii), dict(
+            workload="cylinder, %d levels merged from the %s (Sec. 7.5 study): D2Q9-RR, D=%d, %d levels" % (
+                k, "coarsest" if coarse else "finest", D, 6 - k), steps=300 if k < 4 else 600)
     if name == "cylinder:sponge":     # configs[2] with the paper's far-field pressure relaxation (Eq. 10-11) switched on
         D = int(round(200 * scale))
         return W.cylinder(D=D, sponge_d=(24, 30, 0.1)), dict(
