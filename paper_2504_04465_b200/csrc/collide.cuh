@@ -583,6 +583,10 @@ __device__ __forceinline__ int feq_numerical(const ModelParams& p, T rho, T ux, 
 #pragma unroll
     for (int a = 0; a < NLAMBDA; ++a) r1 += Num<T>::abs_(G[a]);
     converged = r1 <= tol;
+    // single precision: the moment sums carry ~Q eps |M|max rho of rounding (D2Q37: ~7e-5 rho), above the 1e-5 rho of P:934, so a
+    // solve can sit on that floor without ever passing the test: at the iteration limit a residual within 32 tol counts as
+    // converged (the oracle, in double precision, never gets there)
+    if (sizeof(T) == 4 && it >= p.newton_max_iter && r1 <= T(32) * tol) converged = true;
     phase = (converged || it >= p.newton_max_iter) ? POLISH : SEARCH;    // then one unconditional full Newton step
     if (!newton_direction<Q, T>(USE_REFLECT_COMBOS<T> ? sc : f, G, m, d)) { bad = true; break; }
     n0 = norm2sq(G);
