@@ -77,7 +77,7 @@ typedef struct {
   double T0;          /* reference temperature of numerical equilibria; polynomial models use c_s^2 */
   double gamma;       /* specific-heat ratio of the ddf model */
   double sensor_A;    /* Eq. 53 */
-  double newton_tol;
+  double newton_tol;  /* sum_a |G_a| <= newton_tol rho; single precision: within 32 newton_tol at the iteration limit (S27) */
   double bc_rho[4], bc_ux[4], bc_uy[4], bc_T[4];   /* imposed states per side (walls: velocity only) */
   /* Pressure-relaxation sponge against acoustic reflections, Eq. 10-11 P:296-303 (reading S24 of DESIGN.md):
    * sigma(r) = 0 for r < r0, rises linearly to sigma_max at r1 and stays there, r = distance of the cell centre from
