@@ -9,6 +9,8 @@ int kernel_sets_q37(const KernelSet** out) {
   static const KernelSet sets[] = {
       LBM_KSET_MATRIX(37, double, LBM_BGK),
       LBM_KSET_MATRIX(37, double, LBM_RR),
+      LBM_KSET_MATRIX(37, float, LBM_BGK),
+      LBM_KSET_MATRIX(37, float, LBM_RR),
       LBM_KSET_PIPE(37, double, LBM_BGK, true, false),
       LBM_KSET_PIPE(37, double, LBM_BGK, true, true),
       LBM_KSET_PIPE(37, float, LBM_BGK, true, true),

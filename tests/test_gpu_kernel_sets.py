@@ -22,7 +22,7 @@ def _sets():
     for Q in (13, 21):
         out += [(Q, 64, W.BGK, 1, 0), (Q, 64, W.BGK, 1, 1), (Q, 64, W.NUMEQ, 0, 0), (Q, 64, W.NUMEQ, 1, 0), (Q, 64, W.NUMEQ, 1, 1),
                 (Q, 32, W.NUMEQ, 1, 0), (Q, 32, W.NUMEQ, 1, 1)]
-    out += [(37, 64, W.BGK, 0, 0), (37, 64, W.RR, 0, 0), (37, 64, W.BGK, 1, 0), (37, 64, W.BGK, 1, 1), (37, 32, W.BGK, 1, 1),
+    out += [(37, 64, W.BGK, 0, 0), (37, 64, W.RR, 0, 0), (37, 32, W.BGK, 0, 0), (37, 32, W.RR, 0, 0), (37, 64, W.BGK, 1, 0), (37, 64, W.BGK, 1, 1), (37, 32, W.BGK, 1, 1),
             (37, 64, W.NUMEQ, 1, 0), (37, 64, W.NUMEQ, 1, 1), (37, 32, W.NUMEQ, 1, 1)]
     return out
 

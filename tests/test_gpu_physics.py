@@ -79,8 +79,6 @@ def test_taylor_green_decay_rate_through_the_brick_path(lattice, collision, prec
     """exp(-2 nu k^2 t) with nu = c_s^2 (tau - 1/2) (Eq. 3 / P6) on a 512^2 periodic box -- the smallest size that takes the
     regular-brick path by default (2^18 cells) -- for every weakly compressible lattice: the kinetic energy over 4000 steps
     decays at the analytic rate within the O(k^2) lattice error, in fp64 and in fp32."""
-    if lattice == 37 and precision == 32:
-        pytest.skip("the athermal D2Q37 kernels are compiled in fp64 only")
     n, steps = 512, 4000
     case = W.tgv(n, lattice=lattice, collision=collision)
     g = lbm.Grid.from_case(case, precision=precision).bind("cuda:0")
@@ -105,8 +103,6 @@ def test_taylor_green_decay_rate_through_the_matrix_like_path(lattice, collision
     4001 steps (the state ends in the shifted layout), kinetic energy decays at exp(-4 nu k^2 t) within the O(k^2) lattice
     error; mass is conserved to accumulated rounding by the in-place update (4001 steps; D2Q37's 15-digit weights conserve
     to ~1e-14 per collision, S23)."""
-    if lattice == 37 and precision == 32:
-        pytest.skip("the athermal D2Q37 kernels are compiled in fp64 only")
     n, steps = 512, 4001
     case = W.tgv(n, lattice=lattice, collision=collision)
     g = lbm.Grid.from_case(case, precision=precision, addressing=lbm.ADDR_MATRIX).bind("cuda:0")
