@@ -202,8 +202,6 @@ struct lbm_grid {
   int64_t brick_min_cells = BRICK_MIN_LEVEL_CELLS;   // levels below this go through the list (lbm_config.addressing: AUTO)
   bool bricks = false;                            // compressed addressing of regular bricks (off for LBM_ADDR_LIST)
   int device = -1;                                // device of the arena, selected by every entry point for its own duration
-  size_t off_tab = 0;
-  unsigned short* d_tab = nullptr;
   bool pdl = true;                                // programmatic dependent launch between level sweeps (lbm_config.no_pdl)
   bool matrix = false;                            // matrix-like uniform path (matrix.cuh): one population copy, no tables on the device
   size_t off_pos = 0;
@@ -324,7 +322,7 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
   a.tau = g->hg.lv[l].tau;
   a.status = g->d_status;
   a.sigma = L.sigma;
-  a.brick_nb = L.brick_nb; a.brick_tab = g->d_tab; a.irr = L.irr;
+  a.brick_nb = L.brick_nb; a.irr = L.irr;
   a.nbrick = (int)L.nbrick; a.n_irr = (int)L.n_irr;
   a.n_inbox = (int)g->hg.lv[l].n_inbox; a.pf_dist = 0;
   a.queue = (int*)((char*)g->d_status + QUEUE_COUNTER_OFFSET) + 2 * l;
@@ -346,7 +344,8 @@ int enqueue_level(lbm_grid* g, int l, int* cur) {
     a.nbrick = 0; a.brick_ctas = 0; a.irr = nullptr; a.n_irr = (int)L.n;
     a.list_ctas = (int)((L.n + BLOCK - 1) / BLOCK);
     rc = launch_grid(g->ks->sweep_bricks, (unsigned)a.list_ctas, &a, &g->mp, g->launch_stream, g->pdl);
-  } else if (g->bricks && L.nbrick > 0) {
+  } else if (g->bricks && L.nbrick > 0 && (int64_t)g->npop * L.ps < ((int64_t)1 << 32)) {
+    // (brick_update indexes a buffer with 32 bits: a level of 2^32 elements or more per buffer keeps the list kernel)
     rc = launch_grid(g->ks->sweep_bricks, (unsigned)(a.list_ctas + a.brick_ctas), &a, &g->mp, g->launch_stream, g->pdl);
   } else {
     if (L.n >= 4ll * g->pf_dist) a.pf_dist = g->pf_dist;      // smaller levels live in the L2 anyway
@@ -513,7 +512,6 @@ int lbm_grid_create(const lbm_config* cfg, const int64_t* split_off, const int32
       g->updates_per_coarse += H.n << (g->depth - l);
       g->launches_per_coarse += (H.n > 0 ? 1 : 0) * ((int64_t)1 << (g->depth - l));
     }
-    g->off_tab = off; off += round_up(g->hg.brick_tab.size() * 2, ALIGN);
     g->scratch_doubles = (size_t)std::max<int64_t>(4 * g->n_total, nmax * std::max(g->Q, LBM_NLAMBDA)) + 8;
     g->off_scratch = off; off += round_up(g->scratch_doubles * 8, ALIGN);
     g->arena_bytes = off;
@@ -688,8 +686,6 @@ int bind_impl(lbm_grid* g, void* dev_arena, void* cuda_stream) {
     // padding of the population planes is never read by a valid link; zero it once so that exports are clean
     for (int b = 0; b < 2; ++b) CK(cudaMemsetAsync(L.S[b], 0, (size_t)L.ps * g->npop * g->esize, g->stream));
   }
-  g->d_tab = (unsigned short*)(g->arena + g->off_tab);
-  if (!g->matrix) CK(cudaMemcpyAsync(g->d_tab, g->hg.brick_tab.data(), g->hg.brick_tab.size() * 2, cudaMemcpyHostToDevice, g->stream));
   CK(cudaStreamSynchronize(g->stream));
   CK(cudaEventCreate(&g->ev0));
   CK(cudaEventCreate(&g->ev1));

@@ -43,7 +43,6 @@ struct LevelArgs {
   // list (first, so that the slower one-cell-per-thread work is not the tail of the launch), the following brick_ctas
   // CTAs the regular bricks through tile arithmetic
   const int* brick_nb;      // [nbrick][9] first storage index of the 3x3 tiles around (and of, k = 4) the brick
-  const unsigned short* brick_tab;   // [(Q-1)][64] (k << 6) | Z-position of the pull source
   const int* irr;
   int nbrick, n_irr, brick_ctas, list_ctas;
   int n_inbox;              // cells [n_inbox, n) are the boundary cells (Neumann / Dirichlet), the only ones that read aux early
@@ -99,15 +98,17 @@ template <int Q, typename T, int COLL, bool DDF>
 constexpr bool has_bricks = COLL != LBM_NUMEQ;
 
 // Regular-brick path: 64 consecutive cells = one aligned 8x8 tile of fluid cells whose pull sources are
-// base[tile k] + Z-position, (k, Z-position) from a 64-entry table per direction (computed
-// addressing in regular interiors).  Replaces (Q-1) x 4 B of list and the type byte per cell by 36 B per 64 cells.
+// base[tile k] + Z-position (computed addressing in regular interiors).  Replaces (Q-1) x 4 B of
+// list and the type byte per cell by 36 B per 64 cells.
 // Cells of up to 104 bytes of populations (D2Q9/13 in fp64, D2Q9/13/21 in fp32): a thread owns 2 consecutive cells
 // (an x-adjacent pair; 128-bit stores in fp64, 64-bit in fp32), so a brick is one warp (measured: fp64 1 -> 2 cells
 // per thread +7 %; fp32 2 -> 4 cells per thread -3 %, the grid shrinks).  Wider cells (D2Q21 fp64, D2Q37, second
 // distribution) keep one cell per thread (registers); a brick is then two warps.  The 9 tile bases of a brick sit in
-// lanes 0-8 of each of its warps (one coalesced load, issued together with the table loads) and reach the other lanes
-// by shuffle, so the index chain in front of the gathers is one load deep and there is no per-cell index traffic.
-// (Several bricks per warp in sequence, with the table entries loaded once and the next bases prefetched, was measured
+// lanes 0-8 of each of its warps (one coalesced load) and a thread fetches by shuffle the four it can reach; tile and
+// Z-position of a source follow from the thread's (x, y) by arithmetic shared between the directions (round 1 read
+// them from a 64-entry table per direction and shuffled per gather: 113 of the 283 instructions per cell of the fp32
+// D2Q9 kernel went into addressing, profiles/r02_ncu_cylinder_f32.md).  There is no per-cell index traffic.
+// (Several bricks per warp in sequence, with the next bases prefetched, was measured
 // SLOWER: uniform fp64 38.8 against 41.6 GLUPS, the 39 k-cell cavity halves -- the bricks serialise and the grid shrinks.)
 template <int Q, typename T, bool DDF> constexpr int BRICK_CPT = (Q * (DDF ? 2 : 1) * (int)sizeof(T) <= 104) ? 2 : 1;
 template <int Q, typename T, bool DDF> constexpr int brick_cells_per_cta = 128 * BRICK_CPT<Q, T, DDF>;
@@ -123,44 +124,74 @@ __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelPara
   const int brick_raw = (block * 128 + threadIdx.x) / TPB;
   if (brick_raw >= a.nbrick) return;                         // whole warp beyond the last brick
   const int brick = brick_raw;
-  const int m0 = sub * CPT;                                  // Z-position of this thread's first cell
-  const long long ps = a.ps;
-  unsigned e[CPT][(Q + 1) / 3];                              // three 10-bit table entries per register
-#pragma unroll
-  for (int j = 0; j < CPT; ++j) {
-#pragma unroll
-    for (int w = 0; w < (Q + 1) / 3; ++w) e[j][w] = 0u;
-    static_for<1, Q>([&](auto ic) {
-      constexpr int I = decltype(ic)::value;
-      e[j][(I - 1) / 3] |= (unsigned)__ldg(a.brick_tab + (I - 1) * 64 + m0 + j) << (10 * ((I - 1) % 3));
-    });
-  }
+  const int m0 = sub * CPT;                                  // Z-position of this thread's first cell (x in the even bits)
+  // Element index inside a buffer in 32 bits: plane * ps + cell.  lbm_grid_bind sweeps a level through bricks only where
+  // NPOP * ps < 2^32 (every level of every workload here; a wider level keeps the list kernel), so an access is one
+  // three-input add and one IMAD.WIDE against the buffer pointer: no 64-bit plane pointers to form or keep.
+  const unsigned ps32 = (unsigned)a.ps;
+  constexpr int W = Lat<Q>::t.W;
+  // Tile arithmetic (the device form of grid_builder.cpp's table brick_tab, which the host verified against the list):
+  // the pull source of direction i of the cell at (x, y) of the brick is cell (x - cx_i, y - cy_i) mod 8 of the tile
+  // one column / row over where that difference leaves 0..7.  W <= 3 < 4, so a thread reaches at most ONE column
+  // beside the centre (west if x0 < 4, else east) and one row: four tile bases per thread, a select and an add per gather.
+  const int x0 = (m0 & 1) | ((m0 >> 1) & 2) | ((m0 >> 2) & 4), y0 = ((m0 >> 1) & 1) | ((m0 >> 2) & 2) | ((m0 >> 3) & 4);
+  const int kx = x0 < 4 ? 0 : 2, ky = y0 < 4 ? 0 : 6;
   const int nbv = lane < 9 ? __ldg(a.brick_nb + 9ll * brick + lane) : 0;
+  auto spread3 = [](int v) { return (v & 1) | ((v & 2) << 1) | ((v & 4) << 2); };
+  // column terms, by d = (cell of the thread) - cx in [-W, W + CPT - 1]: Z-bits of x0 + d mod 8, and whether x0 + d left the
+  // tile (never for d = 0, nor for d = 1 of an x-adjacent pair: x0 is even there)
+  int colS[2 * W + CPT];
+  bool colP[2 * W + CPT];
+#pragma unroll
+  for (int d = -W; d < W + CPT; ++d) {
+    const int sx = x0 + d;
+    colS[d + W] = d == 0 ? (m0 & 0x15) : (CPT == 2 && d == 1) ? (m0 & 0x15) + 1 : spread3(sx & 7);
+    colP[d + W] = (d < 0 || d >= CPT) && (unsigned)sx > 7u;
+  }
   pdl_wait();
   const T* __restrict__ So = (const T*)a.So;
   T* __restrict__ Sn = (T*)a.Sn;
   const int base = __shfl_sync(0xffffffffu, nbv, grp + 4);
-  T f[CPT][Q], g[CPT][Q], lam[NLAMBDA];
+  const int bXC = __shfl_sync(0xffffffffu, nbv, grp + 3 + kx), bCY = __shfl_sync(0xffffffffu, nbv, grp + 1 + ky);
+  const int bXY = __shfl_sync(0xffffffffu, nbv, grp + kx + ky);
+  // row terms, by cy: first cell of the centre-column / side-column tile of the source row + Z-bits of y0 - cy mod 8
+  int rowC[2 * W + 1], rowX[2 * W + 1];
 #pragma unroll
-  for (int j = 0; j < CPT; ++j) {
-    f[j][0] = So[base + m0 + j];
-    if constexpr (DDF) g[j][0] = So[PL::G0 * ps + base + m0 + j];
-    static_for<1, Q>([&](auto ic) {
-      constexpr int I = decltype(ic)::value;
-      constexpr int SH = 10 * ((I - 1) % 3);
-      const unsigned ent = e[j][(I - 1) / 3];
-      // unsigned 32-bit cell index against a warp-uniform plane pointer: one address instruction per gather
-      const unsigned src = (unsigned)__shfl_sync(0xffffffffu, nbv, grp + (int)((ent >> (SH + 6)) & 15u)) + ((ent >> SH) & 63u);
-      f[j][I] = (So + I * ps)[src];
-      if constexpr (DDF) g[j][I] = (So + (PL::G0 + I) * ps)[src];
-    });
+  for (int cy = -W; cy <= W; ++cy) {
+    const int sy = y0 - cy;
+    const int zy = cy == 0 ? (m0 & 0x2a) : spread3(sy & 7) << 1;
+    const bool py = cy != 0 && (unsigned)sy > 7u;
+    rowC[cy + W] = (py ? bCY : base) + zy;
+    rowX[cy + W] = (py ? bXY : bXC) + zy;
   }
+  T f[CPT][Q], g[CPT][Q], lam[NLAMBDA];
+  static_for<0, Q>([&](auto ic) {
+    constexpr int I = decltype(ic)::value;
+    constexpr int D = -Lat<Q>::t.cx[I], R = Lat<Q>::t.cy[I] + W;
+    if constexpr (CPT == 2 && D == 0) {      // cx = 0: the sources of an x-adjacent pair are adjacent, one address for both
+      const unsigned src = (unsigned)(rowC[R] + colS[W]);
+      const T* qf = So + (src + (unsigned)I * ps32);
+      f[0][I] = qf[0]; f[CPT - 1][I] = qf[1];
+      if constexpr (DDF) {
+        const T* qg = So + (src + (unsigned)(PL::G0 + I) * ps32);
+        g[0][I] = qg[0]; g[CPT - 1][I] = qg[1];
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < CPT; ++j) {
+        const unsigned src = (unsigned)((colP[j + D + W] ? rowX[R] : rowC[R]) + colS[j + D + W]);
+        f[j][I] = So[src + (unsigned)I * ps32];
+        if constexpr (DDF) g[j][I] = So[src + (unsigned)(PL::G0 + I) * ps32];
+      }
+    }
+  });
 #pragma unroll
   for (int j = 0; j < CPT; ++j) {
     T rho;
     collide<Q, T, COLL, DDF, SENSOR>(p, T(a.tau), f[j], g[j], lam, rho);
     if (!(rho > T(0)) || !isfinite(rho)) atomicOr(a.status, FLAG_UNSTABLE);
   }
+  const unsigned dst = (unsigned)(base + m0);
   // a brick starts at any storage index: 128-bit stores when its first cell is CPT-aligned (uniform per brick)
   if (base % CPT == 0) {
 #pragma unroll
@@ -168,11 +199,11 @@ __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelPara
       Vec<T, CPT> o;
 #pragma unroll
       for (int j = 0; j < CPT; ++j) o.v[j] = f[j][i];
-      *reinterpret_cast<Vec<T, CPT>*>(Sn + i * ps + base + m0) = o;
+      *reinterpret_cast<Vec<T, CPT>*>(Sn + (dst + (unsigned)i * ps32)) = o;
       if constexpr (DDF) {
 #pragma unroll
         for (int j = 0; j < CPT; ++j) o.v[j] = g[j][i];
-        *reinterpret_cast<Vec<T, CPT>*>(Sn + (PL::G0 + i) * ps + base + m0) = o;
+        *reinterpret_cast<Vec<T, CPT>*>(Sn + (dst + (unsigned)(PL::G0 + i) * ps32)) = o;
       }
     }
   } else {
@@ -180,8 +211,8 @@ __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelPara
     for (int i = 0; i < Q; ++i)
 #pragma unroll
       for (int j = 0; j < CPT; ++j) {
-        Sn[i * ps + base + m0 + j] = f[j][i];
-        if constexpr (DDF) Sn[(PL::G0 + i) * ps + base + m0 + j] = g[j][i];
+        (Sn + (dst + (unsigned)i * ps32))[j] = f[j][i];
+        if constexpr (DDF) (Sn + (dst + (unsigned)(PL::G0 + i) * ps32))[j] = g[j][i];
       }
   }
 }
