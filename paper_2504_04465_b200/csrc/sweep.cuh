@@ -63,9 +63,21 @@ struct PopLayout {
 template <int Q, typename T, int COLL, bool DDF>
 constexpr int cells_per_thread = (sizeof(T) == 4 && !DDF && COLL != LBM_NUMEQ && Q <= 13) ? 2 : 1;
 
-// Resident CTAs per SM asked of ptxas (register cap): D2Q9 runs at 8 x 128 threads (64 registers).
-template <int Q, typename T, int COLL, bool DDF>
-constexpr int min_ctas_per_sm = (Q == 9 && !DDF && COLL != LBM_NUMEQ) ? 8 : (COLL == LBM_NUMEQ && sizeof(T) == 4 && Q == 13) ? 5 : 1;
+// Resident CTAs per SM asked of ptxas (register cap = 65536 / (128 x CTAs)).  The list kernels: D2Q9 at 8 x 128 threads
+// (64 registers), the fp32 D2Q13 Newton solve at 5.  The brick kernels of the polynomial models are latency-bound (one
+// DRAM round trip per cell, profiles/r02_ncu_cylinder_f32.md: long_scoreboard is the top stall at 50 % of the warps), so
+// they take the occupancy at which the measured throughput peaks, a few spilled bytes included (uniform 4096^2, GLUPS at
+// ptxas' own choice -> here; one step further the spills win and it drops again):
+//   D2Q9  fp32 10 CTAs (48 reg.)  81.2 -> 86.0    D2Q13 fp32 10 (48)  57.1 -> 62.0    D2Q21 fp32 6 (80)  34.7 -> 38.1
+//   D2Q37 fp32  6 (80)  14.2 -> 16.4              D2Q13 fp64  6 (80)  31.5 -> 31.6    D2Q21 fp64 6 (80)  15.9 -> 19.4
+//   D2Q37 fp64  4 (128)  7.7 ->  9.3              D2Q37 + g + sensor fp32 4 (128)  5.3 -> 8.6 (2048^2 Riemann box);
+// its fp64 twin holds 148 registers of populations and loses at 3 CTAs (4.3 -> 3.8), so it stays at ptxas' 2.
+template <int Q, typename T, int COLL, bool DDF, bool BRICKS = false>
+constexpr int min_ctas_per_sm =
+    (BRICKS && !DDF && COLL != LBM_NUMEQ) ? (Q == 9 ? (sizeof(T) == 4 ? 10 : 8) : Q == 13 ? (sizeof(T) == 4 ? 10 : 6) : Q == 21 ? 6 : (sizeof(T) == 4 ? 6 : 4))
+    : (BRICKS && DDF && COLL != LBM_NUMEQ && Q == 37 && sizeof(T) == 4) ? 4
+    : (Q == 9 && !DDF && COLL != LBM_NUMEQ) ? 8
+    : (COLL == LBM_NUMEQ && sizeof(T) == 4 && Q == 13) ? 5 : 1;
 
 template <typename T, int N> struct alignas(sizeof(T) * N) Vec { T v[N]; };
 
@@ -218,7 +230,7 @@ __device__ __forceinline__ void brick_update(const LevelArgs& a, const ModelPara
 }
 
 template <int Q, typename T, int COLL, bool DDF, bool SENSOR, bool BRICKS>
-__global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF>)) sweep_kernel(const LevelArgs a, const ModelParams p) {
+__global__ void __launch_bounds__(128, (min_ctas_per_sm<Q, T, COLL, DDF, BRICKS>)) sweep_kernel(const LevelArgs a, const ModelParams p) {
   using PL = PopLayout<Q, DDF, COLL>;
   constexpr bool NUMEQ = COLL == LBM_NUMEQ;
   constexpr int CPT = BRICKS ? 1 : cells_per_thread<Q, T, COLL, DDF>;
