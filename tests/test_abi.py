@@ -122,6 +122,45 @@ def test_bricks_reproduce_the_oracle_neighbour_list(name):
     g.close()
 
 
+@pytest.mark.parametrize("Q", [9, 13, 21, 37])
+@pytest.mark.parametrize("cpt", [1, 2])
+def test_brick_tile_arithmetic_of_the_device_path(Q, cpt):
+    """The rule brick_update (csrc/sweep.cuh) uses instead of the table, restated here and checked against the table the
+    host builder verified against the list: a thread owning `cpt` x-adjacent cells starting at (x0, y0) of its brick
+    reaches at most one tile column beside the centre (west if x0 < 4, else east) and one tile row, so four tile bases
+    suffice; a source is (crosses the column ? rowX[cy] : rowC[cy]) + colZ[d], d = (cell of the thread) - cx, with no
+    column crossing for d = 0 (nor for d = 1 of a pair: x0 is even there)."""
+    g = lbm.Grid.from_case(W.tgv(32, lattice=Q, collision=W.RR if Q != 37 else W.BGK))
+    cx, cy, w, opp, cs2, reach = O.lattice(Q)
+    assert reach <= 3                                           # W <= 3 < 4: what the one-column / one-row claim rests on
+    _, tab = g.bricks(0)
+    g.close()
+    spread3 = lambda v: (v & 1) | ((v & 2) << 1) | ((v & 4) << 2)
+    for m0 in range(0, 64, cpt):
+        x0, y0 = _zpos(m0)
+        assert cpt == 1 or x0 % 2 == 0
+        kx, ky = (0 if x0 < 4 else 2), (0 if y0 < 4 else 6)
+        # slots of brick_nb[9] (k = column + 3 * row, centre 4) the thread fetches: centre, side column, side row, corner
+        bCC, bXC, bCY, bXY = 4, 3 + kx, 1 + ky, kx + ky
+        for i in range(Q):
+            sy = y0 - int(cy[i])
+            zy = spread3(sy & 7) << 1
+            py = cy[i] != 0 and not (0 <= sy <= 7)
+            rowC, rowX = (bCY if py else bCC), (bXY if py else bXC)
+            for j in range(cpt):
+                d = j - int(cx[i])
+                sx = x0 + d
+                px = (d < 0 or d >= cpt) and not (0 <= sx <= 7)
+                if not (d < 0 or d >= cpt):
+                    assert 0 <= sx <= 7                         # the static no-crossing cases
+                k, z = (rowX if px else rowC), zy + spread3(sx & 7)
+                if i == 0:
+                    assert (k, z) == (4, m0 + j)
+                else:
+                    e = int(tab[i - 1, m0 + j])
+                    assert (k, z) == (e >> 6, e & 63), (Q, cpt, m0, j, i)
+
+
 def test_brick_coverage_of_the_bench_shapes():
     """A periodic uniform box is all bricks; the graded cylinder mesh is mostly bricks on its fine levels."""
     g = lbm.Grid.from_case(W.tgv(64))
